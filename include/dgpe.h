@@ -1,0 +1,126 @@
+/*
+ * dgpe.h -- C-ABI boundary of libdgpe: the split-step Crank-Nicolson (SSCN) time step of the
+ * 3-D dipolar Gross-Pitaevskii equation on one NVIDIA B200 (sm_100a), complex fp64.
+ *
+ * Citations: P:Lnn = /root/reference/PAPER.md line nn (arXiv:1610.05329); BJ = BASELINE.json
+ * (north_star, configs[i]); R#n = reading n of DESIGN.md section 3.
+ *
+ * The method ("Gross-Pitaevskii equation with contact and dipolar interaction in a harmonic
+ * anisotropic trap"; "split-step Crank-Nicolson method ... imaginary or real time ... The
+ * contribution of the dipolar interaction is evaluated by a Fourier transformation to momentum
+ * space using a convolution theorem"; P:L39 real-to-complex transform of the density):
+ *
+ *   i dpsi/dt = [ -1/2 lap + 1/2 (gamma^2 x^2 + nu^2 y^2 + lambda^2 z^2) + g |psi|^2 + gdd Phi ] psi,
+ *   Phi = Udd * |psi|^2,   Udd~(k) = (4 pi/3)(3 kz^2/|k|^2 - 1),  Udd~(0) = 0      (BJ:configs[0]),
+ *   imaginary time: t -> -i tau, renormalised to  sum |psi|^2 dx dy dz = 1  after every step.
+ *
+ * One step (BJ:north_star (a)-(d)):
+ *   (a) Phi = IFFT[ Udd~(k) FFT(|psi|^2) ];
+ *   (b) psi <- exp(-i dt H) psi (real time) or exp(-dt H) psi (imaginary time), H = V + g|psi|^2 + gdd Phi;
+ *   (c) three Crank-Nicolson line sweeps (x, y, z), Dirichlet psi = 0 on the end nodes of every axis;
+ *   (d) imaginary time only: psi <- psi / sqrt(sum |psi|^2 dV).
+ *
+ * Layout: psi is complex double (re, im interleaved, 16 bytes per point), row-major
+ * [nx][ny][nz], NX the slowest and NZ the contiguous dimension; x_i = (i - nx/2) dx (R#6).
+ *
+ * Memory: every `psi` argument is a DEVICE pointer to nx*ny*nz complex doubles, 16-byte aligned,
+ * owned by the caller (e.g. a contiguous torch.complex128 CUDA tensor); the library never allocates
+ * or frees it.  Every `double*` result argument is a HOST pointer.  The handle owns all device
+ * workspace (half-spectrum buffer, per-axis tables, reduction scratch) and is immutable after
+ * creation: a parameter quench is a second handle (BJ:configs[2]).
+ *
+ * Errors ("programs will test if these conditions are met, and inform the user"):
+ * dgpe_create returns NULL, every other call returns a negative DGPE_ERR_* code, and
+ * dgpe_last_error() returns a thread-local, human-readable description.  There is no CPU fallback.
+ */
+#ifndef DGPE_H
+#define DGPE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dgpe_handle dgpe_handle;
+
+enum { DGPE_IMAG = 0, DGPE_REAL = 1 };
+
+enum {
+    DGPE_OK = 0,
+    DGPE_ERR_ARG = -1,       /* bad argument (see dgpe_create)                               */
+    DGPE_ERR_CUDA = -2,      /* a CUDA runtime call or kernel launch failed                  */
+    DGPE_ERR_NOMEM = -3,     /* host or device allocation failed                             */
+    DGPE_ERR_UNSUPPORTED = -4, /* size outside what the kernels support                      */
+    DGPE_ERR_NONFINITE = -5  /* imaginary time: the norm became 0, inf or NaN during the call */
+};
+
+/*
+ * dgpe_create -- build a handle for one grid and one set of physical parameters.
+ *   nx, ny, nz   grid points per axis; each >= 4, of the form 2^a 3^b (P:L130 FFT-friendly sizes,
+ *                radix 2 and 3 built), <= DGPE_MAX_N; nz even (the R2C half-spectrum, R#13).
+ *   dx, dy, dz   grid spacings  (> 0);  dt  time step (> 0).
+ *   gamma, nu, lambda   trap frequencies along x, y, z (R#2: gamma<->x slowest, lambda<->z).
+ *   g, gdd       contact and dipolar interaction strengths; dipoles polarised along z (R#2).
+ *   mode         DGPE_IMAG or DGPE_REAL.
+ * Returns NULL on error (DGPE_ERR_ARG / UNSUPPORTED / NOMEM / CUDA in dgpe_last_error()).
+ * Uses the current CUDA device; allocates 16*nx*ny*(nz/2+1) bytes plus O(nx+ny+nz) tables.
+ */
+#define DGPE_MAX_N 1024
+dgpe_handle* dgpe_create(int nx, int ny, int nz, double dx, double dy, double dz, double dt,
+                         double gamma, double nu, double lambda, double g, double gdd, int mode);
+
+/* Frees the handle's device and host memory.  NULL is allowed. */
+void dgpe_destroy(dgpe_handle* h);
+
+/* All later work of this handle is enqueued on `cuda_stream` (a cudaStream_t passed as void*;
+   NULL = the legacy default stream, which is also the initial setting). */
+int dgpe_set_stream(dgpe_handle* h, void* cuda_stream);
+
+/*
+ * dgpe_step -- advance psi in place by nsteps full SSCN steps (BJ:north_star (a)-(d)).
+ * All kernels are enqueued on the handle's stream without host synchronisation inside the loop.
+ * Imaginary time: the per-step renormalisation (d) is carried as a scalar into the next step's
+ * kernels and applied explicitly once at the end, so psi has unit norm on return; the call then
+ * waits for the stream and returns DGPE_ERR_NONFINITE if a norm was 0/inf/NaN (R#18: no clamp).
+ * Real time: psi is never rescaled; the call returns after enqueueing.
+ * nsteps = 0 is a no-op.  Errors: DGPE_ERR_ARG (NULL, nsteps < 0), DGPE_ERR_CUDA.
+ */
+int dgpe_step(dgpe_handle* h, void* psi, int nsteps);
+
+/* Observables (R#14-R#17).  Each call enqueues on the handle's stream, waits for it and writes HOST
+   doubles.  psi need not be normalised; mu, E and rms are divided by the norm.
+     norm   = sum |psi|^2 dx dy dz                               (the integral, not its root)
+     mu     = [T + sum(V n + g n^2 + gdd Phi n) dV] / norm
+     energy = [T + sum(V n + g n^2/2 + gdd Phi n/2) dV] / norm
+     T      = sum_axes 1/2 sum_links |psi_{j+1} - psi_j|^2 / d^2 dV,  links j = -1..n-1, psi_-1 = psi_n = 0
+     rms    = { sqrt<x^2>, sqrt<y^2>, sqrt<z^2>, sqrt<x^2+y^2+z^2> }  about the origin            */
+int dgpe_norm(dgpe_handle* h, const void* psi, double* norm);
+int dgpe_chempot(dgpe_handle* h, const void* psi, double* mu);
+int dgpe_energy(dgpe_handle* h, const void* psi, double* energy);
+int dgpe_rms(dgpe_handle* h, const void* psi, double rms[4]);
+/* out[0] = T, out[1] = <V>, out[2] = g<n>, out[3] = gdd<Phi>, each divided by the norm
+   (mu = sum of the four; energy = out0 + out1 + out2/2 + out3/2). */
+int dgpe_energy_terms(dgpe_handle* h, const void* psi, double out[4]);
+
+/* Stage entry points (diagnostics and per-stage parity tests; same kernels as dgpe_step):
+     dgpe_dipolar    phi (DEVICE, nx*ny*nz doubles) <- Phi of step (a) for the given psi
+     dgpe_nonlinear  psi <- steps (a)+(b) only
+     dgpe_sweep      psi <- one Crank-Nicolson sweep of step (c) along axis 0 = x, 1 = y, 2 = z   */
+int dgpe_dipolar(dgpe_handle* h, const void* psi, void* phi);
+int dgpe_nonlinear(dgpe_handle* h, void* psi);
+int dgpe_sweep(dgpe_handle* h, void* psi, int axis);
+
+/* Waits for the handle's stream. */
+int dgpe_synchronize(dgpe_handle* h);
+
+/* Algorithmic bytes one step moves (model of the kernels as built) and the
+   number of kernel launches per step; used by bench.py for the roofline line. */
+double dgpe_bytes_per_step(const dgpe_handle* h);
+int dgpe_launches_per_step(const dgpe_handle* h);
+
+/* Thread-local description of the last error ("" if none). Never NULL. */
+const char* dgpe_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,147 @@
+"""ctypes binding of libdgpe.so -- the C-ABI of include/dgpe.h, same names, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/; there is no CPU fallback: if the built
+library or a CUDA device is missing, the calls raise.  torch is used for device memory and streams.
+"""
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+IMAG, REAL = 0, 1
+OK, ERR_ARG, ERR_CUDA, ERR_NOMEM, ERR_UNSUPPORTED, ERR_NONFINITE = 0, -1, -2, -3, -4, -5
+
+EXPORTS = ("dgpe_create", "dgpe_destroy", "dgpe_set_stream", "dgpe_step", "dgpe_norm", "dgpe_chempot",
+           "dgpe_energy", "dgpe_rms", "dgpe_energy_terms", "dgpe_dipolar", "dgpe_nonlinear", "dgpe_sweep",
+           "dgpe_synchronize", "dgpe_bytes_per_step", "dgpe_launches_per_step", "dgpe_last_error")
+
+_lib = None
+
+
+class DgpeError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"dgpe error {code}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load (building if needed) paper_1610_05329_b200/libdgpe.so.  Raises if it cannot be built/loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        vp, dp, ci, cd = C.c_void_p, C.POINTER(C.c_double), C.c_int, C.c_double
+        L.dgpe_create.restype = vp
+        L.dgpe_create.argtypes = [ci, ci, ci, cd, cd, cd, cd, cd, cd, cd, cd, cd, ci]
+        L.dgpe_destroy.restype = None
+        L.dgpe_destroy.argtypes = [vp]
+        L.dgpe_set_stream.argtypes = [vp, vp]
+        L.dgpe_step.argtypes = [vp, vp, ci]
+        for name in ("dgpe_norm", "dgpe_chempot", "dgpe_energy", "dgpe_rms", "dgpe_energy_terms"):
+            getattr(L, name).argtypes = [vp, vp, dp]
+        L.dgpe_dipolar.argtypes = [vp, vp, vp]
+        L.dgpe_nonlinear.argtypes = [vp, vp]
+        L.dgpe_sweep.argtypes = [vp, vp, ci]
+        L.dgpe_synchronize.argtypes = [vp]
+        L.dgpe_bytes_per_step.restype = cd
+        L.dgpe_bytes_per_step.argtypes = [vp]
+        L.dgpe_launches_per_step.argtypes = [vp]
+        L.dgpe_last_error.restype = C.c_char_p
+        L.dgpe_last_error.argtypes = []
+        _lib = L
+    return _lib
+
+
+def last_error():
+    return lib().dgpe_last_error().decode()
+
+
+def _check(rc):
+    if rc != OK:
+        raise DgpeError(rc, last_error())
+
+
+class Dgpe:
+    """One dgpe_handle.  psi arguments are contiguous torch.complex128 CUDA tensors of shape (nx, ny, nz)."""
+
+    def __init__(self, nx, ny, nz, dx, dy, dz, dt, gamma, nu, lam, g, gdd, mode, stream=None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1610_05329_b200 needs a CUDA device (no CPU fallback)")
+        self.shape = (nx, ny, nz)
+        self.mode = mode
+        self.h = lib().dgpe_create(nx, ny, nz, dx, dy, dz, dt, gamma, nu, lam, g, gdd, mode)
+        if not self.h:
+            raise DgpeError(ERR_ARG, last_error())
+        self.set_stream(stream if stream is not None else torch.cuda.current_stream())
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().dgpe_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_stream(self, stream):
+        ptr = stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream or 0)
+        _check(lib().dgpe_set_stream(self.h, C.c_void_p(ptr)))
+
+    def _psi(self, psi):
+        if not (isinstance(psi, torch.Tensor) and psi.is_cuda and psi.dtype == torch.complex128
+                and psi.is_contiguous() and tuple(psi.shape) == self.shape):
+            raise TypeError(f"psi must be a contiguous CUDA complex128 tensor of shape {self.shape}")
+        return C.c_void_p(psi.data_ptr())
+
+    def step(self, psi, nsteps=1):
+        """dgpe_step; returns the status code (OK or ERR_NONFINITE), raises on every other error."""
+        rc = lib().dgpe_step(self.h, self._psi(psi), int(nsteps))
+        if rc not in (OK, ERR_NONFINITE):
+            _check(rc)
+        return rc
+
+    def _scalars(self, fn, psi, n):
+        out = (C.c_double * n)()
+        _check(fn(self.h, self._psi(psi), out))
+        return out[0] if n == 1 else [out[i] for i in range(n)]
+
+    def norm(self, psi):
+        return self._scalars(lib().dgpe_norm, psi, 1)
+
+    def chempot(self, psi):
+        return self._scalars(lib().dgpe_chempot, psi, 1)
+
+    def energy(self, psi):
+        return self._scalars(lib().dgpe_energy, psi, 1)
+
+    def rms(self, psi):
+        return self._scalars(lib().dgpe_rms, psi, 4)
+
+    def energy_terms(self, psi):
+        return self._scalars(lib().dgpe_energy_terms, psi, 4)
+
+    def dipolar(self, psi):
+        phi = torch.empty(self.shape, dtype=torch.float64, device=psi.device)
+        _check(lib().dgpe_dipolar(self.h, self._psi(psi), C.c_void_p(phi.data_ptr())))
+        return phi
+
+    def nonlinear(self, psi):
+        _check(lib().dgpe_nonlinear(self.h, self._psi(psi)))
+
+    def sweep(self, psi, axis):
+        _check(lib().dgpe_sweep(self.h, self._psi(psi), int(axis)))
+
+    def synchronize(self):
+        _check(lib().dgpe_synchronize(self.h))
+
+    @property
+    def bytes_per_step(self):
+        return lib().dgpe_bytes_per_step(self.h)
+
+    @property
+    def launches_per_step(self):
+        return lib().dgpe_launches_per_step(self.h)

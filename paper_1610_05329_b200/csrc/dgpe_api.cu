@@ -1,0 +1,645 @@
+// dgpe_api.cu -- host side of libdgpe: the C-ABI of include/dgpe.h, the handle (plans, per-axis
+// tables, workspace) and the kernel launches of one SSCN step.  No CPU implementation of any stage
+// lives here: without a CUDA device every call fails.
+#include "../../include/dgpe.h"
+
+#include <algorithm>
+#include <cmath>
+#include <complex>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "common.cuh"
+#include "fft.cuh"
+#include "observe.cuh"
+#include "spectral.cuh"
+#include "sweep.cuh"
+
+using namespace dgpe;
+
+// ------------------------------------------------------------------------------------------------
+// errors
+// ------------------------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(e_ == cudaErrorMemoryAllocation ? DGPE_ERR_NOMEM : DGPE_ERR_CUDA,          \
+                        "%s failed: %s", #call, cudaGetErrorString(e_));                           \
+    } while (0)
+
+extern "C" const char* dgpe_last_error(void) { return g_err; }
+
+// ------------------------------------------------------------------------------------------------
+// handle
+// ------------------------------------------------------------------------------------------------
+struct AxisSweep {
+    int n = 0, Lc = 0, G = 0, Kf = 0, Kb = 0;
+    std::complex<double> r;
+    void* inv = nullptr;   // device tables, double (imag) or cplx (real)
+    void* cc = nullptr;
+    void* F = nullptr;
+    void* Gm = nullptr;
+    void* Ach = nullptr;
+    void* Bch = nullptr;
+};
+
+struct dgpe_handle {
+    int nx, ny, nz, nzh, mode;
+    double dx, dy, dz, dt, gamma, nu, lambda, g, gdd;
+    long long N;
+    cudaStream_t stream = nullptr;
+
+    cplx* spec = nullptr;                       // [nx][ny][nzh]
+    FftPlan plan_x{}, plan_y{}, plan_zh{};      // transform lengths nx, ny, nz/2
+    cplx *tw_x = nullptr, *tw_y = nullptr, *tw_zh = nullptr, *tw_split = nullptr;
+    double *kx2 = nullptr, *ky2 = nullptr, *kz2 = nullptr;
+    double *vx = nullptr, *vy = nullptr, *vz = nullptr;      // gamma^2 x^2, nu^2 y^2, lambda^2 z^2
+    double *x2 = nullptr, *y2 = nullptr, *z2 = nullptr;      // squared coordinates
+    AxisSweep sw[3];
+    double* scal = nullptr;          // device scalars (SC_*)
+    double* partials = nullptr;
+    unsigned int* ticket = nullptr;
+    double* d_out = nullptr;         // device results (16 doubles)
+    double* h_out = nullptr;         // pinned host mirror
+    std::vector<void*> owned;        // everything to cudaFree
+};
+
+static int threads_for(int nbf)
+{
+    int t = nbf * TILE_COLS;
+    return ((t + 31) / 32) * 32;
+}
+
+template <typename T>
+static int upload(dgpe_handle* h, const std::vector<T>& v, T** out)
+{
+    T* d = nullptr;
+    CU(cudaMalloc(&d, sizeof(T) * (v.empty() ? 1 : v.size())));
+    h->owned.push_back(d);
+    if (!v.empty()) CU(cudaMemcpy(d, v.data(), sizeof(T) * v.size(), cudaMemcpyHostToDevice));
+    *out = d;
+    return DGPE_OK;
+}
+
+static bool smooth23(int n)
+{
+    if (n < 1) return false;
+    while (n % 2 == 0) n /= 2;
+    while (n % 3 == 0) n /= 3;
+    return n == 1;
+}
+
+// radices 8, 4, 2 first, 3 last; butterfly slots per column = n / largest radix
+static int make_plan(dgpe_handle* h, int n, FftPlan* P, cplx** tw_dev)
+{
+    std::memset(P, 0, sizeof(*P));
+    P->n = n;
+    int m = n, np = 0, rmax = 1;
+    const int order[4] = {8, 4, 2, 3};
+    for (int oi = 0; oi < 4; ++oi) {
+        const int R = order[oi];
+        while (m % R == 0 && m > 1) {
+            if (np >= MAX_PASSES) return fail(DGPE_ERR_UNSUPPORTED, "FFT length %d needs too many passes", n);
+            P->radix[np++] = R;
+            m /= R;
+            if (R > rmax) rmax = R;
+        }
+    }
+    if (m != 1) return fail(DGPE_ERR_ARG, "FFT length %d is not of the form 2^a 3^b", n);
+    if (np == 0) {           // n == 1: one radix-1 "pass" does not exist; callers never ask for it
+        return fail(DGPE_ERR_ARG, "FFT length %d too small", n);
+    }
+    P->npass = np;
+    P->nbf = n / rmax;
+    for (int p = 0; p < np; ++p) {
+        const int nbut = n / P->radix[p];
+        P->nb[p] = (nbut + P->nbf - 1) / P->nbf;
+    }
+    std::vector<cplx> tw(n);
+    const long double TWO_PI = 6.283185307179586476925286766559005768L;
+    for (int j = 0; j < n; ++j) {
+        long double a = TWO_PI * (long double)j / (long double)n;
+        tw[j] = make_double2((double)cosl(a), (double)(-sinl(a)));
+    }
+    int rc = upload(h, tw, tw_dev);
+    P->tw = *tw_dev;
+    return rc;
+}
+
+// wave number of DFT bin m (R#10, R#11): k = 2 pi f/(n d), f = m for m <= n/2, else m - n
+static std::vector<double> wavenum_sq(int n, double d, int count)
+{
+    const double PI = 3.14159265358979323846264338327950288;
+    std::vector<double> v(count);
+    for (int m = 0; m < count; ++m) {
+        int f = (m <= n / 2) ? m : m - n;
+        double k = 2.0 * PI * (double)f / ((double)n * d);
+        v[m] = k * k;
+    }
+    return v;
+}
+
+template <typename CT>
+static CT to_ct(std::complex<double> z);
+template <>
+double to_ct<double>(std::complex<double> z) { return z.real(); }
+template <>
+cplx to_ct<cplx>(std::complex<double> z) { return make_double2(z.real(), z.imag()); }
+
+template <typename CT>
+static int build_sweep(dgpe_handle* h, AxisSweep* S, int n, std::complex<double> r)
+{
+    typedef std::complex<double> C;
+    S->n = n;
+    S->r = r;
+    S->Lc = 16;
+    const int nun = n - 2;
+    S->G = (nun + S->Lc - 1) / S->Lc;
+    std::vector<C> inv(n, C(0)), cc(n, C(0)), F(n, C(0)), Gm(n, C(0)), A(S->G, C(0)), B(S->G, C(0));
+    const C diag = 1.0 + 2.0 * r;
+    inv[1] = 1.0 / diag;
+    cc[1] = -r * inv[1];
+    for (int j = 2; j <= n - 2; ++j) {
+        inv[j] = 1.0 / (diag + r * cc[j - 1]);
+        cc[j] = -r * inv[j];
+    }
+    double amax = 0.0, bmax = 0.0;
+    for (int g = 0; g < S->G; ++g) {
+        const int s = 1 + g * S->Lc, t = std::min(s + S->Lc, n - 1);
+        C acc = 1.0;
+        for (int j = s; j < t; ++j) { acc *= r * inv[j]; F[j] = acc; }
+        A[g] = acc;
+        acc = 1.0;
+        for (int j = t - 1; j >= s; --j) { acc *= -cc[j]; Gm[j] = acc; }
+        B[g] = acc;
+        amax = std::max(amax, std::abs(A[g]));
+        bmax = std::max(bmax, std::abs(B[g]));
+    }
+    const double tol = std::ldexp(1.0, -80);
+    auto depth = [&](double q) {
+        int K = 1;
+        double p = q;
+        while (K < S->G && p > tol) { p *= q; ++K; }
+        return K;
+    };
+    S->Kf = depth(amax);
+    S->Kb = depth(bmax);
+    auto conv = [&](const std::vector<C>& v, void** out) -> int {
+        std::vector<CT> w(v.size());
+        for (size_t i = 0; i < v.size(); ++i) w[i] = to_ct<CT>(v[i]);
+        CT* d = nullptr;
+        int rc = upload(h, w, &d);
+        *out = d;
+        return rc;
+    };
+    int rc;
+    if ((rc = conv(inv, &S->inv))) return rc;
+    if ((rc = conv(cc, &S->cc))) return rc;
+    if ((rc = conv(F, &S->F))) return rc;
+    if ((rc = conv(Gm, &S->Gm))) return rc;
+    if ((rc = conv(A, &S->Ach))) return rc;
+    if ((rc = conv(B, &S->Bch))) return rc;
+    return DGPE_OK;
+}
+
+static size_t sweep_smem(int n, int G, bool zaxis)
+{
+    return sizeof(cplx) * ((size_t)n * (zaxis ? 9 : 8) + 2 * (size_t)G * TILE_COLS);
+}
+
+template <typename K>
+static int allow_smem(K kernel, size_t bytes)
+{
+    if (bytes > 227 * 1024) return fail(DGPE_ERR_UNSUPPORTED, "tile needs %zu bytes of shared memory", bytes);
+    CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return DGPE_OK;
+}
+
+static int init_handle(dgpe_handle* h)
+{
+    const int nx = h->nx, ny = h->ny, nz = h->nz, nzh = h->nzh, M = nz / 2;
+    int rc;
+    int dev_count = 0;
+    CU(cudaGetDeviceCount(&dev_count));
+    if (dev_count < 1) return fail(DGPE_ERR_CUDA, "no CUDA device");
+
+    if ((rc = make_plan(h, nx, &h->plan_x, &h->tw_x))) return rc;
+    if ((rc = make_plan(h, ny, &h->plan_y, &h->tw_y))) return rc;
+    if ((rc = make_plan(h, M, &h->plan_zh, &h->tw_zh))) return rc;
+    {
+        std::vector<cplx> tw(M + 1);
+        const long double TWO_PI = 6.283185307179586476925286766559005768L;
+        for (int k = 0; k <= M; ++k) {
+            long double a = TWO_PI * (long double)k / (long double)nz;
+            tw[k] = make_double2((double)cosl(a), (double)(-sinl(a)));
+        }
+        if ((rc = upload(h, tw, &h->tw_split))) return rc;
+    }
+    if ((rc = upload(h, wavenum_sq(nx, h->dx, nx), &h->kx2))) return rc;
+    if ((rc = upload(h, wavenum_sq(ny, h->dy, ny), &h->ky2))) return rc;
+    if ((rc = upload(h, wavenum_sq(nz, h->dz, nzh), &h->kz2))) return rc;
+
+    auto coord_tables = [&](int n, double d, double om, double** v, double** c2) -> int {
+        std::vector<double> tv(n), tc(n);
+        for (int i = 0; i < n; ++i) {
+            double x = (double)(i - n / 2) * d;      // R#6
+            tv[i] = om * om * x * x;
+            tc[i] = x * x;
+        }
+        int r1 = upload(h, tv, v);
+        if (r1) return r1;
+        return upload(h, tc, c2);
+    };
+    if ((rc = coord_tables(nx, h->dx, h->gamma, &h->vx, &h->x2))) return rc;
+    if ((rc = coord_tables(ny, h->dy, h->nu, &h->vy, &h->y2))) return rc;
+    if ((rc = coord_tables(nz, h->dz, h->lambda, &h->vz, &h->z2))) return rc;
+
+    const int ns[3] = {nx, ny, nz};
+    const double ds[3] = {h->dx, h->dy, h->dz};
+    for (int a = 0; a < 3; ++a) {
+        const double rr = h->dt / (4.0 * ds[a] * ds[a]);      // R#9
+        if (h->mode == DGPE_IMAG)
+            rc = build_sweep<double>(h, &h->sw[a], ns[a], std::complex<double>(rr, 0.0));
+        else
+            rc = build_sweep<cplx>(h, &h->sw[a], ns[a], std::complex<double>(0.0, rr));
+        if (rc) return rc;
+    }
+
+    CU(cudaMalloc(&h->spec, sizeof(cplx) * (size_t)nx * ny * nzh));
+    h->owned.push_back(h->spec);
+    size_t nblk = std::max({(size_t)(((long long)ny * nz + 7) / 8), (size_t)nx * ((nz + 7) / 8),
+                            (size_t)(((long long)nx * ny + 7) / 8), (size_t)4096});
+    CU(cudaMalloc(&h->partials, sizeof(double) * nblk * MAX_RED));
+    h->owned.push_back(h->partials);
+    CU(cudaMalloc(&h->ticket, sizeof(unsigned int)));
+    h->owned.push_back(h->ticket);
+    CU(cudaMemset(h->ticket, 0, sizeof(unsigned int)));
+    CU(cudaMalloc(&h->scal, sizeof(double) * SC_COUNT));
+    h->owned.push_back(h->scal);
+    {
+        double init[SC_COUNT] = {1.0, 1.0, 1.0, 0.0, 0, 0, 0, 0};
+        CU(cudaMemcpy(h->scal, init, sizeof(init), cudaMemcpyHostToDevice));
+    }
+    CU(cudaMalloc(&h->d_out, sizeof(double) * 16));
+    h->owned.push_back(h->d_out);
+    CU(cudaMallocHost(&h->h_out, sizeof(double) * 16));
+
+    // shared-memory opt-in for every kernel that may exceed 48 KB
+    const size_t fft_xy = sizeof(cplx) * TILE_COLS * (size_t)std::max(nx, ny);
+    const size_t fft_z = sizeof(cplx) * TILE_COLS * (size_t)(M + 1);
+    if ((rc = allow_smem(k_fft_lines<false, 512>, fft_xy))) return rc;
+    if ((rc = allow_smem(k_fft_lines<true, 512>, fft_xy))) return rc;
+    if ((rc = allow_smem(k_fft_lines<false, 1024>, fft_xy))) return rc;
+    if ((rc = allow_smem(k_fft_lines<true, 1024>, fft_xy))) return rc;
+    if ((rc = allow_smem(k_fft_x_udd<512>, fft_xy))) return rc;
+    if ((rc = allow_smem(k_fft_x_udd<1024>, fft_xy))) return rc;
+    if ((rc = allow_smem(k_dens_r2c, fft_z))) return rc;
+    if ((rc = allow_smem(k_c2r_nonlin<0>, fft_z))) return rc;
+    if ((rc = allow_smem(k_c2r_nonlin<1>, fft_z))) return rc;
+    if ((rc = allow_smem(k_c2r_nonlin<2>, fft_z))) return rc;
+    if ((rc = allow_smem(k_c2r_nonlin<3>, fft_z))) return rc;
+    size_t sxy = std::max(sweep_smem(nx, h->sw[0].G, false), sweep_smem(ny, h->sw[1].G, false));
+    size_t sz = sweep_smem(nz, h->sw[2].G, true);
+    if (h->mode == DGPE_IMAG) {
+        if ((rc = allow_smem(k_sweep<double, false>, sxy))) return rc;
+        if ((rc = allow_smem(k_sweep<double, true>, sz))) return rc;
+    } else {
+        if ((rc = allow_smem(k_sweep<cplx, false>, sxy))) return rc;
+        if ((rc = allow_smem(k_sweep<cplx, true>, sz))) return rc;
+    }
+    return DGPE_OK;
+}
+
+extern "C" dgpe_handle* dgpe_create(int nx, int ny, int nz, double dx, double dy, double dz, double dt,
+                                    double gamma, double nu, double lambda, double g, double gdd, int mode)
+{
+    g_err[0] = 0;
+    const int ns[3] = {nx, ny, nz};
+    for (int a = 0; a < 3; ++a) {
+        if (ns[a] < 4) { fail(DGPE_ERR_ARG, "grid size %d < 4", ns[a]); return nullptr; }
+        if (!smooth23(ns[a])) { fail(DGPE_ERR_ARG, "grid size %d is not of the form 2^a 3^b", ns[a]); return nullptr; }
+        if (ns[a] > DGPE_MAX_N) { fail(DGPE_ERR_UNSUPPORTED, "grid size %d > %d", ns[a], DGPE_MAX_N); return nullptr; }
+    }
+    if (nz % 2) { fail(DGPE_ERR_ARG, "nz = %d must be even", nz); return nullptr; }
+    if (!(dx > 0.0) || !(dy > 0.0) || !(dz > 0.0) || !(dt > 0.0) || !std::isfinite(dx) || !std::isfinite(dy) ||
+        !std::isfinite(dz) || !std::isfinite(dt)) {
+        fail(DGPE_ERR_ARG, "dx, dy, dz, dt must be positive and finite");
+        return nullptr;
+    }
+    if (mode != DGPE_IMAG && mode != DGPE_REAL) { fail(DGPE_ERR_ARG, "mode %d is neither DGPE_IMAG nor DGPE_REAL", mode); return nullptr; }
+    dgpe_handle* h = new (std::nothrow) dgpe_handle();
+    if (!h) { fail(DGPE_ERR_NOMEM, "host allocation failed"); return nullptr; }
+    h->nx = nx; h->ny = ny; h->nz = nz; h->nzh = nz / 2 + 1; h->mode = mode;
+    h->dx = dx; h->dy = dy; h->dz = dz; h->dt = dt;
+    h->gamma = gamma; h->nu = nu; h->lambda = lambda; h->g = g; h->gdd = gdd;
+    h->N = (long long)nx * ny * nz;
+    if (init_handle(h) != DGPE_OK) {
+        char keep[sizeof(g_err)];
+        std::memcpy(keep, g_err, sizeof(keep));
+        dgpe_destroy(h);
+        std::memcpy(g_err, keep, sizeof(keep));
+        return nullptr;
+    }
+    return h;
+}
+
+extern "C" void dgpe_destroy(dgpe_handle* h)
+{
+    if (!h) return;
+    cudaStreamSynchronize(h->stream);
+    for (void* p : h->owned) cudaFree(p);
+    if (h->h_out) cudaFreeHost(h->h_out);
+    delete h;
+}
+
+extern "C" int dgpe_set_stream(dgpe_handle* h, void* cuda_stream)
+{
+    if (!h) return fail(DGPE_ERR_ARG, "NULL handle");
+    h->stream = (cudaStream_t)cuda_stream;
+    return DGPE_OK;
+}
+
+extern "C" int dgpe_synchronize(dgpe_handle* h)
+{
+    if (!h) return fail(DGPE_ERR_ARG, "NULL handle");
+    CU(cudaStreamSynchronize(h->stream));
+    return DGPE_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// launches
+// ------------------------------------------------------------------------------------------------
+static int check_launch(const char* what)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(DGPE_ERR_CUDA, "launch of %s failed: %s", what, cudaGetErrorString(e));
+    return DGPE_OK;
+}
+
+// K1..K4: spec <- Udd~(k)/N * FFT(s2 |psi|^2), transformed back along x and y
+static int launch_dipolar_spectrum(dgpe_handle* h, const cplx* psi)
+{
+    const int nx = h->nx, ny = h->ny, nz = h->nz, nzh = h->nzh, M = nz / 2;
+    const int nlines = nx * ny;
+    int rc;
+    k_dens_r2c<<<(nlines + 7) / 8, threads_for(h->plan_zh.nbf), sizeof(cplx) * TILE_COLS * (size_t)M, h->stream>>>(
+        psi, h->spec, nlines, nz, h->plan_zh, h->tw_split, h->scal);
+    if ((rc = check_launch("k_dens_r2c"))) return rc;
+
+    LineMap my{ny, nzh, (long long)ny * nzh, 1, nzh};
+    dim3 gy((nzh + 7) / 8, nx);
+    const int ty = threads_for(h->plan_y.nbf), tx = threads_for(h->plan_x.nbf);
+    const size_t smy = sizeof(cplx) * TILE_COLS * (size_t)ny, smx = sizeof(cplx) * TILE_COLS * (size_t)nx;
+    if (ty <= 512)
+        k_fft_lines<false, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+    else
+        k_fft_lines<false, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+    if ((rc = check_launch("k_fft_lines<fwd,y>"))) return rc;
+
+    LineMap mx{nx, ny * nzh, 0, 1, (long long)ny * nzh};
+    if (tx <= 512)
+        k_fft_x_udd<512><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
+                                                                     1.0 / (double)h->N);
+    else
+        k_fft_x_udd<1024><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
+                                                                      1.0 / (double)h->N);
+    if ((rc = check_launch("k_fft_x_udd"))) return rc;
+
+    if (ty <= 512)
+        k_fft_lines<true, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+    else
+        k_fft_lines<true, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+    return check_launch("k_fft_lines<inv,y>");
+}
+
+// K5 in one of its modes
+static int launch_c2r(dgpe_handle* h, cplx* psi, int kmode, double* out)
+{
+    const int nlines = h->nx * h->ny, M = h->nz / 2;
+    NonlinArgs A;
+    A.nlines = nlines; A.ny = h->ny; A.nz = h->nz;
+    A.dt = h->dt; A.g = h->g; A.gdd = h->gdd;
+    A.vx = h->vx; A.vy = h->vy; A.vz = h->vz;
+    A.scal = h->scal; A.partials = h->partials; A.ticket = h->ticket; A.out = out;
+    const int grid = (nlines + 7) / 8, thr = threads_for(h->plan_zh.nbf);
+    const size_t sm = sizeof(cplx) * TILE_COLS * (size_t)(M + 1);
+    switch (kmode) {
+        case 0: k_c2r_nonlin<0><<<grid, thr, sm, h->stream>>>(psi, h->spec, h->plan_zh, h->tw_split, A); break;
+        case 1: k_c2r_nonlin<1><<<grid, thr, sm, h->stream>>>(psi, h->spec, h->plan_zh, h->tw_split, A); break;
+        case 2: k_c2r_nonlin<2><<<grid, thr, sm, h->stream>>>(psi, h->spec, h->plan_zh, h->tw_split, A); break;
+        default: k_c2r_nonlin<3><<<grid, thr, sm, h->stream>>>(psi, h->spec, h->plan_zh, h->tw_split, A); break;
+    }
+    return check_launch("k_c2r_nonlin");
+}
+
+template <typename CT>
+static int launch_sweep_t(dgpe_handle* h, cplx* psi, int axis, bool fold)
+{
+    const AxisSweep& S = h->sw[axis];
+    const int nx = h->nx, ny = h->ny, nz = h->nz;
+    SweepTables<CT> T;
+    T.r = to_ct<CT>(S.r);
+    T.omr2 = to_ct<CT>(1.0 - 2.0 * S.r);
+    T.inv = (const CT*)S.inv; T.cc = (const CT*)S.cc; T.F = (const CT*)S.F; T.Gm = (const CT*)S.Gm;
+    T.Ach = (const CT*)S.Ach; T.Bch = (const CT*)S.Bch;
+    T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb;
+    SweepFold F;
+    F.enabled = fold ? 1 : 0;
+    F.dV = h->dx * h->dy * h->dz;
+    F.partials = h->partials; F.ticket = h->ticket; F.scal = h->scal;
+    const int thr = threads_for(S.G);
+    if (axis == 0) {
+        LineMap m{nx, ny * nz, 0, 1, (long long)ny * nz};
+        k_sweep<CT, false><<<(ny * nz + 7) / 8, thr, sweep_smem(nx, S.G, false), h->stream>>>(psi, m, T, F);
+    } else if (axis == 1) {
+        LineMap m{ny, nz, (long long)ny * nz, 1, nz};
+        dim3 grid((nz + 7) / 8, nx);
+        k_sweep<CT, false><<<grid, thr, sweep_smem(ny, S.G, false), h->stream>>>(psi, m, T, F);
+    } else {
+        LineMap m{nz, nx * ny, 0, nz, 1};
+        k_sweep<CT, true><<<(nx * ny + 7) / 8, thr, sweep_smem(nz, S.G, true), h->stream>>>(psi, m, T, F);
+    }
+    return check_launch("k_sweep");
+}
+
+static int launch_sweep(dgpe_handle* h, cplx* psi, int axis, bool fold)
+{
+    return h->mode == DGPE_IMAG ? launch_sweep_t<double>(h, psi, axis, fold) : launch_sweep_t<cplx>(h, psi, axis, fold);
+}
+
+static int set_scal(dgpe_handle* h, int clear_bad)
+{
+    k_set_scal<<<1, 1, 0, h->stream>>>(h->scal, 1.0, 1.0, clear_bad);
+    return check_launch("k_set_scal");
+}
+
+extern "C" int dgpe_step(dgpe_handle* h, void* psi_, int nsteps)
+{
+    if (!h || !psi_) return fail(DGPE_ERR_ARG, "NULL handle or psi");
+    if (nsteps < 0) return fail(DGPE_ERR_ARG, "nsteps = %d < 0", nsteps);
+    if (nsteps == 0) return DGPE_OK;
+    cplx* psi = (cplx*)psi_;
+    const bool imag = h->mode == DGPE_IMAG;
+    int rc;
+    if ((rc = set_scal(h, 1))) return rc;
+    for (int s = 0; s < nsteps; ++s) {
+        if ((rc = launch_dipolar_spectrum(h, psi))) return rc;
+        if ((rc = launch_c2r(h, psi, imag ? 0 : 1, nullptr))) return rc;
+        if ((rc = launch_sweep(h, psi, 0, false))) return rc;
+        if ((rc = launch_sweep(h, psi, 1, false))) return rc;
+        if ((rc = launch_sweep(h, psi, 2, imag))) return rc;
+    }
+    if (imag) {
+        k_scale<<<148 * 8, 256, 0, h->stream>>>(psi, h->N, h->scal);
+        if ((rc = check_launch("k_scale"))) return rc;
+        CU(cudaMemcpyAsync(h->h_out, h->scal, sizeof(double) * SC_COUNT, cudaMemcpyDeviceToHost, h->stream));
+        if ((rc = set_scal(h, 0))) return rc;
+        CU(cudaStreamSynchronize(h->stream));
+        if (h->h_out[SC_BAD] != 0.0)
+            return fail(DGPE_ERR_NONFINITE, "imaginary-time norm became zero or non-finite (last norm %g)", h->h_out[SC_NORM]);
+    }
+    return DGPE_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// stage entry points
+// ------------------------------------------------------------------------------------------------
+extern "C" int dgpe_dipolar(dgpe_handle* h, const void* psi, void* phi)
+{
+    if (!h || !psi || !phi) return fail(DGPE_ERR_ARG, "NULL argument");
+    int rc;
+    if ((rc = launch_dipolar_spectrum(h, (const cplx*)psi))) return rc;
+    return launch_c2r(h, const_cast<cplx*>((const cplx*)psi), 3, (double*)phi);
+}
+
+extern "C" int dgpe_nonlinear(dgpe_handle* h, void* psi)
+{
+    if (!h || !psi) return fail(DGPE_ERR_ARG, "NULL argument");
+    int rc;
+    if ((rc = launch_dipolar_spectrum(h, (const cplx*)psi))) return rc;
+    return launch_c2r(h, (cplx*)psi, h->mode == DGPE_IMAG ? 0 : 1, nullptr);
+}
+
+extern "C" int dgpe_sweep(dgpe_handle* h, void* psi, int axis)
+{
+    if (!h || !psi) return fail(DGPE_ERR_ARG, "NULL argument");
+    if (axis < 0 || axis > 2) return fail(DGPE_ERR_ARG, "axis %d not in 0..2", axis);
+    return launch_sweep(h, (cplx*)psi, axis, false);
+}
+
+// ------------------------------------------------------------------------------------------------
+// observables
+// ------------------------------------------------------------------------------------------------
+static ObsArgs obs_args(dgpe_handle* h, double* out)
+{
+    ObsArgs A;
+    A.nx = h->nx; A.ny = h->ny; A.nz = h->nz;
+    A.x2 = h->x2; A.y2 = h->y2; A.z2 = h->z2;
+    A.partials = h->partials; A.ticket = h->ticket; A.out = out;
+    return A;
+}
+
+static int fetch(dgpe_handle* h, int count)
+{
+    CU(cudaMemcpyAsync(h->h_out, h->d_out, sizeof(double) * count, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return DGPE_OK;
+}
+
+static int moments(dgpe_handle* h, const void* psi)
+{
+    const int grid = std::min(h->nx * h->ny, 148 * 8);
+    k_moments<<<grid, 256, 0, h->stream>>>((const cplx*)psi, obs_args(h, h->d_out));
+    int rc = check_launch("k_moments");
+    if (rc) return rc;
+    return fetch(h, 4);
+}
+
+extern "C" int dgpe_norm(dgpe_handle* h, const void* psi, double* norm)
+{
+    if (!h || !psi || !norm) return fail(DGPE_ERR_ARG, "NULL argument");
+    int rc = moments(h, psi);
+    if (rc) return rc;
+    *norm = h->h_out[0] * h->dx * h->dy * h->dz;
+    return DGPE_OK;
+}
+
+extern "C" int dgpe_rms(dgpe_handle* h, const void* psi, double rms[4])
+{
+    if (!h || !psi || !rms) return fail(DGPE_ERR_ARG, "NULL argument");
+    int rc = moments(h, psi);
+    if (rc) return rc;
+    const double s = h->h_out[0];
+    rms[0] = std::sqrt(h->h_out[1] / s);
+    rms[1] = std::sqrt(h->h_out[2] / s);
+    rms[2] = std::sqrt(h->h_out[3] / s);
+    rms[3] = std::sqrt((h->h_out[1] + h->h_out[2] + h->h_out[3]) / s);
+    return DGPE_OK;
+}
+
+extern "C" int dgpe_energy_terms(dgpe_handle* h, const void* psi, double out[4])
+{
+    if (!h || !psi || !out) return fail(DGPE_ERR_ARG, "NULL argument");
+    int rc;
+    if ((rc = launch_dipolar_spectrum(h, (const cplx*)psi))) return rc;
+    if ((rc = launch_c2r(h, const_cast<cplx*>((const cplx*)psi), 2, h->d_out))) return rc;
+    const int grid = std::min(h->nx * h->ny, 148 * 8);
+    k_kinetic<<<grid, 256, 0, h->stream>>>((const cplx*)psi, obs_args(h, h->d_out + 4));
+    if ((rc = check_launch("k_kinetic"))) return rc;
+    if ((rc = fetch(h, 8))) return rc;
+    const double sV = h->h_out[0], sg = h->h_out[1], sdd = h->h_out[2], s = h->h_out[3];
+    const double T = 0.5 * (h->h_out[4] / (h->dx * h->dx) + h->h_out[5] / (h->dy * h->dy) + h->h_out[6] / (h->dz * h->dz));
+    out[0] = T / s;
+    out[1] = sV / s;
+    out[2] = h->g * sg / s;
+    out[3] = h->gdd * sdd / s;
+    return DGPE_OK;
+}
+
+extern "C" int dgpe_chempot(dgpe_handle* h, const void* psi, double* mu)
+{
+    if (!mu) return fail(DGPE_ERR_ARG, "NULL argument");
+    double t[4];
+    int rc = dgpe_energy_terms(h, psi, t);
+    if (rc) return rc;
+    *mu = t[0] + t[1] + t[2] + t[3];
+    return DGPE_OK;
+}
+
+extern "C" int dgpe_energy(dgpe_handle* h, const void* psi, double* energy)
+{
+    if (!energy) return fail(DGPE_ERR_ARG, "NULL argument");
+    double t[4];
+    int rc = dgpe_energy_terms(h, psi, t);
+    if (rc) return rc;
+    *energy = t[0] + t[1] + 0.5 * t[2] + 0.5 * t[3];
+    return DGPE_OK;
+}
+
+extern "C" double dgpe_bytes_per_step(const dgpe_handle* h)
+{
+    if (!h) return 0.0;
+    const double N = (double)h->N, S = 16.0 * (double)h->nx * h->ny * h->nzh;
+    // K1 16N+S, K2 2S, K3 2S, K4 2S, K5 S+32N, three sweeps 32N each (model M1)
+    return 144.0 * N + 8.0 * S;
+}
+
+extern "C" int dgpe_launches_per_step(const dgpe_handle* h)
+{
+    (void)h;
+    return 8;
+}

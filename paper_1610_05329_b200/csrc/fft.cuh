@@ -1,0 +1,176 @@
+// fft.cuh -- mixed-radix (2, 3, 4, 8) Stockham autosort FFT passes over a shared-memory tile of
+// TILE_COLS lines (FFT-friendly sizes 2^a 3^b ...; BJ:north_star "mixed-radix (2^a 3^b)
+// shared-memory Stockham FFT passes per axis").
+//
+// Pass p of an n-point transform with radix R and Ns = product of the radices of the passes before it:
+//   for every butterfly j in [0, n/R):   k = j mod Ns
+//     v_q  = in[j + q n/R] * w_n^{q k n/(Ns R)}                 q = 0..R-1
+//     out[(j div Ns) Ns R + k + s Ns] = sum_q v_q w_R^{q s}     s = 0..R-1
+// w_n = exp(-2 pi i/n) forward, exp(+2 pi i/n) inverse; no normalisation.
+//
+// Thread layout: thread = (c, b), c = tid & 7 the tile column (line), b = tid >> 3 the butterfly slot.
+// A quarter-warp (8 lanes, one 128-byte shared-memory wavefront of a 16-byte access) is the 8 columns
+// of ONE tile row, so every access pattern along the transform index is bank-conflict free.
+// Passes run in place: each thread holds its NB butterflies (NB*R values) in registers across the
+// barrier that separates the reads of a pass from its writes.
+#pragma once
+#include "common.cuh"
+
+namespace dgpe {
+
+template <bool INV>
+__device__ __forceinline__ cplx mul_w4(cplx a)   // * w_4 = -i (forward) or +i (inverse)
+{
+    return INV ? mul_pi(a) : mul_mi(a);
+}
+
+template <int R, bool INV>
+struct Butterfly;
+
+template <bool INV>
+struct Butterfly<2, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[2])
+    {
+        cplx a = v[0], b = v[1];
+        v[0] = cadd(a, b);
+        v[1] = csub(a, b);
+    }
+};
+
+template <bool INV>
+struct Butterfly<3, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[3])
+    {
+        const double S = 0.86602540378443864676372317075294;   // sin(pi/3)
+        cplx t1 = cadd(v[1], v[2]);
+        cplx m1 = mk(v[0].x - 0.5 * t1.x, v[0].y - 0.5 * t1.y);
+        cplx df = cscale(csub(v[1], v[2]), S);
+        cplx m2 = mul_w4<INV>(df);                              // -i S (v1 - v2) forward
+        v[0] = cadd(v[0], t1);
+        v[1] = cadd(m1, m2);
+        v[2] = csub(m1, m2);
+    }
+};
+
+template <bool INV>
+struct Butterfly<4, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[4])
+    {
+        cplx t0 = cadd(v[0], v[2]), t1 = csub(v[0], v[2]);
+        cplx t2 = cadd(v[1], v[3]), t3 = mul_w4<INV>(csub(v[1], v[3]));
+        v[0] = cadd(t0, t2);
+        v[1] = cadd(t1, t3);
+        v[2] = csub(t0, t2);
+        v[3] = csub(t1, t3);
+    }
+};
+
+template <bool INV>
+struct Butterfly<8, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[8])
+    {
+        const double H = 0.70710678118654752440084436210485;   // sqrt(1/2)
+        cplx e[4] = {v[0], v[2], v[4], v[6]};
+        cplx o[4] = {v[1], v[3], v[5], v[7]};
+        Butterfly<4, INV>::run(e);
+        Butterfly<4, INV>::run(o);
+        // w_8^1 = (1 -/+ i)/sqrt2, w_8^2 = -/+ i, w_8^3 = (-1 -/+ i)/sqrt2   (forward / inverse)
+        cplx o1 = INV ? mk((o[1].x - o[1].y) * H, (o[1].x + o[1].y) * H)
+                      : mk((o[1].x + o[1].y) * H, (o[1].y - o[1].x) * H);
+        cplx o2 = mul_w4<INV>(o[2]);
+        cplx o3 = INV ? mk((-o[3].x - o[3].y) * H, (o[3].x - o[3].y) * H)
+                      : mk((o[3].y - o[3].x) * H, (-o[3].x - o[3].y) * H);
+        v[0] = cadd(e[0], o[0]);
+        v[4] = csub(e[0], o[0]);
+        v[1] = cadd(e[1], o1);
+        v[5] = csub(e[1], o1);
+        v[2] = cadd(e[2], o2);
+        v[6] = csub(e[2], o2);
+        v[3] = cadd(e[3], o3);
+        v[7] = csub(e[3], o3);
+    }
+};
+
+// One pass.  src/dst are generic pointers (shared or global) already offset to this thread's column;
+// sstride/dstride = elements between consecutive transform indices.  `active` masks the columns of a
+// ragged last tile; every thread of the block must call (two block barriers inside).
+template <int R, int NB, bool INV>
+__device__ __noinline__ void fft_pass(int n, int Ns, int b, int nbf, bool active,
+                                         const cplx* src, long long sstride,
+                                         cplx* dst, long long dstride,
+                                         const cplx* __restrict__ tw)
+{
+    const int nbut = n / R;
+    const int twstep = n / (Ns * R);
+    cplx v[NB][R];
+#pragma unroll
+    for (int u = 0; u < NB; ++u) {
+        const int j = b + u * nbf;
+        if (active && j < nbut) {
+            const int k = j % Ns;
+#pragma unroll
+            for (int q = 0; q < R; ++q) v[u][q] = src[(long long)(j + q * nbut) * sstride];
+            if (Ns > 1) {
+#pragma unroll
+                for (int q = 1; q < R; ++q) {
+                    cplx w = __ldg(&tw[q * k * twstep]);
+                    if (INV) w.y = -w.y;
+                    v[u][q] = cmul(v[u][q], w);
+                }
+            }
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int u = 0; u < NB; ++u) {
+        const int j = b + u * nbf;
+        if (active && j < nbut) {
+            Butterfly<R, INV>::run(v[u]);
+            const int k = j % Ns;
+            const int base = (j / Ns) * Ns * R + k;
+#pragma unroll
+            for (int s = 0; s < R; ++s) dst[(long long)(base + s * Ns) * dstride] = v[u][s];
+        }
+    }
+    __syncthreads();
+}
+
+// All passes of one transform.  The first pass reads `src` (stride sstride), the last writes `dst`
+// (stride dstride); everything in between goes through the shared-memory tile `sm` (stride smstride).
+// src and/or dst may be the tile itself.
+template <bool INV>
+__device__ __forceinline__ void fft_run(const FftPlan& P, int b, bool active,
+                                        const cplx* src, long long sstride,
+                                        cplx* sm, long long smstride,
+                                        cplx* dst, long long dstride)
+{
+    int Ns = 1;
+    for (int p = 0; p < P.npass; ++p) {
+        const cplx* s = (p == 0) ? src : sm;
+        const long long ss = (p == 0) ? sstride : smstride;
+        cplx* d = (p == P.npass - 1) ? dst : sm;
+        const long long ds = (p == P.npass - 1) ? dstride : smstride;
+        const int R = P.radix[p];
+#define DGPE_PASS(RR, NN)                                                                     \
+    case (RR * 8 + NN):                                                                        \
+        fft_pass<RR, NN, INV>(P.n, Ns, b, P.nbf, active, s, ss, d, ds, P.tw);                  \
+        break;
+        switch (R * 8 + P.nb[p]) {
+            DGPE_PASS(8, 1)
+            DGPE_PASS(4, 1)
+            DGPE_PASS(4, 2)
+            DGPE_PASS(3, 1)
+            DGPE_PASS(3, 2)
+            DGPE_PASS(3, 3)
+            DGPE_PASS(2, 1)
+            DGPE_PASS(2, 2)
+            DGPE_PASS(2, 3)
+            DGPE_PASS(2, 4)
+            default: break;
+        }
+#undef DGPE_PASS
+        Ns *= R;
+    }
+}
+
+}  // namespace dgpe
