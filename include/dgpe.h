@@ -109,6 +109,25 @@ int dgpe_dipolar(dgpe_handle* h, const void* psi, void* phi);
 int dgpe_nonlinear(dgpe_handle* h, void* psi);
 int dgpe_sweep(dgpe_handle* h, void* psi, int axis);
 
+/*
+ * dgpe_step_host -- the same as dgpe_step for a wave function in HOST memory: copies nx*ny*nz complex
+ * doubles from psi_host (pinned memory makes the copies asynchronous DMA; pageable memory works, slower)
+ * to a device buffer the handle owns (allocated on first use, 16*nx*ny*nz bytes), runs nsteps steps,
+ * copies the result back into psi_host and waits for the stream.  Same return codes as dgpe_step,
+ * plus DGPE_ERR_NOMEM if the staging buffer cannot be allocated.
+ */
+int dgpe_step_host(dgpe_handle* h, void* psi_host, int nsteps);
+
+/*
+ * dgpe_step_profile -- run nsteps steps exactly as dgpe_step does, with a CUDA event recorded on the
+ * handle's stream between consecutive kernels; ms[k] (HOST, dgpe_launches_per_step() doubles) receives
+ * the average duration in milliseconds of kernel k of the step.  Waits for the stream.
+ * dgpe_kernel_name(k) / dgpe_kernel_bytes(h, k) give the name and the algorithmic bytes of kernel k.
+ */
+int dgpe_step_profile(dgpe_handle* h, void* psi, int nsteps, double* ms);
+const char* dgpe_kernel_name(const dgpe_handle* h, int k);
+double dgpe_kernel_bytes(const dgpe_handle* h, int k);
+
 /* Waits for the handle's stream. */
 int dgpe_synchronize(dgpe_handle* h);
 

@@ -15,6 +15,7 @@ OK, ERR_ARG, ERR_CUDA, ERR_NOMEM, ERR_UNSUPPORTED, ERR_NONFINITE = 0, -1, -2, -3
 
 EXPORTS = ("dgpe_create", "dgpe_destroy", "dgpe_set_stream", "dgpe_step", "dgpe_norm", "dgpe_chempot",
            "dgpe_energy", "dgpe_rms", "dgpe_energy_terms", "dgpe_dipolar", "dgpe_nonlinear", "dgpe_sweep",
+           "dgpe_step_host", "dgpe_step_profile", "dgpe_kernel_name", "dgpe_kernel_bytes",
            "dgpe_synchronize", "dgpe_bytes_per_step", "dgpe_launches_per_step", "dgpe_last_error")
 
 _lib = None
@@ -44,6 +45,12 @@ def lib():
         L.dgpe_dipolar.argtypes = [vp, vp, vp]
         L.dgpe_nonlinear.argtypes = [vp, vp]
         L.dgpe_sweep.argtypes = [vp, vp, ci]
+        L.dgpe_step_host.argtypes = [vp, vp, ci]
+        L.dgpe_step_profile.argtypes = [vp, vp, ci, dp]
+        L.dgpe_kernel_name.restype = C.c_char_p
+        L.dgpe_kernel_name.argtypes = [vp, ci]
+        L.dgpe_kernel_bytes.restype = cd
+        L.dgpe_kernel_bytes.argtypes = [vp, ci]
         L.dgpe_synchronize.argtypes = [vp]
         L.dgpe_bytes_per_step.restype = cd
         L.dgpe_bytes_per_step.argtypes = [vp]
@@ -103,6 +110,26 @@ class Dgpe:
         if rc not in (OK, ERR_NONFINITE):
             _check(rc)
         return rc
+
+    def step_host(self, psi_host, nsteps=1):
+        """dgpe_step_host on a contiguous CPU complex128 tensor (pinned for full-speed copies)."""
+        if not (isinstance(psi_host, torch.Tensor) and not psi_host.is_cuda and psi_host.dtype == torch.complex128
+                and psi_host.is_contiguous() and tuple(psi_host.shape) == self.shape):
+            raise TypeError(f"psi_host must be a contiguous CPU complex128 tensor of shape {self.shape}")
+        rc = lib().dgpe_step_host(self.h, C.c_void_p(psi_host.data_ptr()), int(nsteps))
+        if rc not in (OK, ERR_NONFINITE):
+            _check(rc)
+        return rc
+
+    def step_profile(self, psi, nsteps=1):
+        """dgpe_step_profile: list of (kernel name, algorithmic bytes, average ms) for the kernels of a step."""
+        nk = self.launches_per_step
+        ms = (C.c_double * nk)()
+        rc = lib().dgpe_step_profile(self.h, self._psi(psi), int(nsteps), ms)
+        if rc not in (OK, ERR_NONFINITE):
+            _check(rc)
+        return [(lib().dgpe_kernel_name(self.h, k).decode(), lib().dgpe_kernel_bytes(self.h, k), ms[k])
+                for k in range(nk)]
 
     def _scalars(self, fn, psi, n):
         out = (C.c_double * n)()

@@ -75,6 +75,8 @@ struct dgpe_handle {
     unsigned int* ticket = nullptr;
     double* d_out = nullptr;         // device results (16 doubles)
     double* h_out = nullptr;         // pinned host mirror
+    cplx* psi_stage = nullptr;       // dgpe_step_host: device copy of psi (lazy)
+    std::vector<cudaEvent_t> prof_ev; // dgpe_step_profile
     std::vector<void*> owned;        // everything to cudaFree
 };
 
@@ -363,6 +365,7 @@ extern "C" void dgpe_destroy(dgpe_handle* h)
     cudaStreamSynchronize(h->stream);
     for (void* p : h->owned) cudaFree(p);
     if (h->h_out) cudaFreeHost(h->h_out);
+    for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
     delete h;
 }
 
@@ -487,32 +490,174 @@ static int set_scal(dgpe_handle* h, int clear_bad)
     return check_launch("k_set_scal");
 }
 
+// One step = 8 kernels.  `mark`, if set, is called after each launch with the kernel index.
+static const char* const KERNEL_NAMES[8] = {"K1 dens_r2c(z)", "K2 fft_y fwd", "K3 fft_x*Udd*ifft_x", "K4 fft_y inv",
+                                            "K5 c2r(z)+nonlinear", "K6 sweep_x", "K7 sweep_y", "K8 sweep_z(+norm)"};
+
+template <typename Mark>
+static int one_step(dgpe_handle* h, cplx* psi, Mark mark)
+{
+    const bool imag = h->mode == DGPE_IMAG;
+    const int nx = h->nx, ny = h->ny, nz = h->nz, nzh = h->nzh, M = nz / 2;
+    const int nlines = nx * ny;
+    int rc;
+    // K1
+    k_dens_r2c<<<(nlines + 7) / 8, threads_for(h->plan_zh.nbf), sizeof(cplx) * TILE_COLS * (size_t)M, h->stream>>>(
+        psi, h->spec, nlines, nz, h->plan_zh, h->tw_split, h->scal);
+    if ((rc = check_launch("k_dens_r2c"))) return rc;
+    mark(0);
+    // K2
+    LineMap my{ny, nzh, (long long)ny * nzh, 1, nzh};
+    dim3 gy((nzh + 7) / 8, nx);
+    const int ty = threads_for(h->plan_y.nbf), tx = threads_for(h->plan_x.nbf);
+    const size_t smy = sizeof(cplx) * TILE_COLS * (size_t)ny, smx = sizeof(cplx) * TILE_COLS * (size_t)nx;
+    if (ty <= 512)
+        k_fft_lines<false, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+    else
+        k_fft_lines<false, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+    if ((rc = check_launch("k_fft_lines<fwd,y>"))) return rc;
+    mark(1);
+    // K3
+    LineMap mx{nx, ny * nzh, 0, 1, (long long)ny * nzh};
+    if (tx <= 512)
+        k_fft_x_udd<512><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
+                                                                     1.0 / (double)h->N);
+    else
+        k_fft_x_udd<1024><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
+                                                                      1.0 / (double)h->N);
+    if ((rc = check_launch("k_fft_x_udd"))) return rc;
+    mark(2);
+    // K4
+    if (ty <= 512)
+        k_fft_lines<true, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+    else
+        k_fft_lines<true, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+    if ((rc = check_launch("k_fft_lines<inv,y>"))) return rc;
+    mark(3);
+    // K5
+    if ((rc = launch_c2r(h, psi, imag ? 0 : 1, nullptr))) return rc;
+    mark(4);
+    // K6..K8
+    if ((rc = launch_sweep(h, psi, 0, false))) return rc;
+    mark(5);
+    if ((rc = launch_sweep(h, psi, 1, false))) return rc;
+    mark(6);
+    if ((rc = launch_sweep(h, psi, 2, imag))) return rc;
+    mark(7);
+    return DGPE_OK;
+}
+
+static int finish_steps(dgpe_handle* h, cplx* psi)
+{
+    int rc;
+    k_scale<<<148 * 8, 256, 0, h->stream>>>(psi, h->N, h->scal);
+    if ((rc = check_launch("k_scale"))) return rc;
+    CU(cudaMemcpyAsync(h->h_out, h->scal, sizeof(double) * SC_COUNT, cudaMemcpyDeviceToHost, h->stream));
+    return set_scal(h, 0);
+}
+
+static int check_finite(dgpe_handle* h)
+{
+    if (h->h_out[SC_BAD] != 0.0)
+        return fail(DGPE_ERR_NONFINITE, "imaginary-time norm became zero or non-finite (last norm %g)", h->h_out[SC_NORM]);
+    return DGPE_OK;
+}
+
 extern "C" int dgpe_step(dgpe_handle* h, void* psi_, int nsteps)
 {
     if (!h || !psi_) return fail(DGPE_ERR_ARG, "NULL handle or psi");
     if (nsteps < 0) return fail(DGPE_ERR_ARG, "nsteps = %d < 0", nsteps);
     if (nsteps == 0) return DGPE_OK;
     cplx* psi = (cplx*)psi_;
-    const bool imag = h->mode == DGPE_IMAG;
+    int rc;
+    if ((rc = set_scal(h, 1))) return rc;
+    for (int s = 0; s < nsteps; ++s)
+        if ((rc = one_step(h, psi, [](int) {}))) return rc;
+    if (h->mode == DGPE_IMAG) {
+        if ((rc = finish_steps(h, psi))) return rc;
+        CU(cudaStreamSynchronize(h->stream));
+        return check_finite(h);
+    }
+    return DGPE_OK;
+}
+
+extern "C" int dgpe_step_host(dgpe_handle* h, void* psi_host, int nsteps)
+{
+    if (!h || !psi_host) return fail(DGPE_ERR_ARG, "NULL handle or psi");
+    if (nsteps < 0) return fail(DGPE_ERR_ARG, "nsteps = %d < 0", nsteps);
+    const size_t bytes = sizeof(cplx) * (size_t)h->N;
+    if (!h->psi_stage) {
+        CU(cudaMalloc(&h->psi_stage, bytes));
+        h->owned.push_back(h->psi_stage);
+    }
+    CU(cudaMemcpyAsync(h->psi_stage, psi_host, bytes, cudaMemcpyHostToDevice, h->stream));
+    int rc;
+    bool imag_done = false;
+    if (nsteps > 0) {
+        if ((rc = set_scal(h, 1))) return rc;
+        for (int s = 0; s < nsteps; ++s)
+            if ((rc = one_step(h, h->psi_stage, [](int) {}))) return rc;
+        if (h->mode == DGPE_IMAG) {
+            if ((rc = finish_steps(h, h->psi_stage))) return rc;
+            imag_done = true;
+        }
+    }
+    CU(cudaMemcpyAsync(psi_host, h->psi_stage, bytes, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return imag_done ? check_finite(h) : DGPE_OK;
+}
+
+extern "C" int dgpe_step_profile(dgpe_handle* h, void* psi_, int nsteps, double* ms)
+{
+    if (!h || !psi_ || !ms) return fail(DGPE_ERR_ARG, "NULL argument");
+    if (nsteps < 1) return fail(DGPE_ERR_ARG, "nsteps = %d < 1", nsteps);
+    const int NK = dgpe_launches_per_step(h);
+    const size_t need = (size_t)nsteps * (NK + 1);
+    while (h->prof_ev.size() < need) {
+        cudaEvent_t e;
+        CU(cudaEventCreate(&e));
+        h->prof_ev.push_back(e);
+    }
+    cplx* psi = (cplx*)psi_;
     int rc;
     if ((rc = set_scal(h, 1))) return rc;
     for (int s = 0; s < nsteps; ++s) {
-        if ((rc = launch_dipolar_spectrum(h, psi))) return rc;
-        if ((rc = launch_c2r(h, psi, imag ? 0 : 1, nullptr))) return rc;
-        if ((rc = launch_sweep(h, psi, 0, false))) return rc;
-        if ((rc = launch_sweep(h, psi, 1, false))) return rc;
-        if ((rc = launch_sweep(h, psi, 2, imag))) return rc;
+        cudaEvent_t* ev = &h->prof_ev[(size_t)s * (NK + 1)];
+        cudaEventRecord(ev[0], h->stream);
+        cudaStream_t st = h->stream;
+        if ((rc = one_step(h, psi, [ev, st](int k) { cudaEventRecord(ev[k + 1], st); }))) return rc;
     }
-    if (imag) {
-        k_scale<<<148 * 8, 256, 0, h->stream>>>(psi, h->N, h->scal);
-        if ((rc = check_launch("k_scale"))) return rc;
-        CU(cudaMemcpyAsync(h->h_out, h->scal, sizeof(double) * SC_COUNT, cudaMemcpyDeviceToHost, h->stream));
-        if ((rc = set_scal(h, 0))) return rc;
-        CU(cudaStreamSynchronize(h->stream));
-        if (h->h_out[SC_BAD] != 0.0)
-            return fail(DGPE_ERR_NONFINITE, "imaginary-time norm became zero or non-finite (last norm %g)", h->h_out[SC_NORM]);
+    if (h->mode == DGPE_IMAG && (rc = finish_steps(h, psi))) return rc;
+    CU(cudaStreamSynchronize(h->stream));
+    for (int k = 0; k < NK; ++k) ms[k] = 0.0;
+    for (int s = 0; s < nsteps; ++s) {
+        cudaEvent_t* ev = &h->prof_ev[(size_t)s * (NK + 1)];
+        for (int k = 0; k < NK; ++k) {
+            float t = 0.f;
+            CU(cudaEventElapsedTime(&t, ev[k], ev[k + 1]));
+            ms[k] += (double)t / nsteps;
+        }
     }
-    return DGPE_OK;
+    return h->mode == DGPE_IMAG ? check_finite(h) : DGPE_OK;
+}
+
+extern "C" const char* dgpe_kernel_name(const dgpe_handle* h, int k)
+{
+    (void)h;
+    return (k >= 0 && k < 8) ? KERNEL_NAMES[k] : "";
+}
+
+extern "C" double dgpe_kernel_bytes(const dgpe_handle* h, int k)
+{
+    if (!h) return 0.0;
+    const double N = (double)h->N, S = 16.0 * (double)h->nx * h->ny * h->nzh;
+    switch (k) {
+        case 0: return 16.0 * N + S;       // read psi, write half-spectrum
+        case 1: case 2: case 3: return 2.0 * S;
+        case 4: return S + 32.0 * N;       // read spectrum, read + write psi
+        case 5: case 6: case 7: return 32.0 * N;
+        default: return 0.0;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------

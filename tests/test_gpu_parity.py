@@ -1,0 +1,320 @@
+"""GPU parity tests proper (-m gpu): the CUDA path, called through the C-ABI (ctypes binding), against
+the CPU oracle on the same seeded inputs, element by element; and at BASELINE.json's full sizes via
+sampled lines the oracle solves one by one and closed forms that hold at any size.
+
+Tolerances (BJ:north_star): max|psi_gpu - psi_ref| <= 1e-12 after one step, <= 1e-10 after 100 steps;
+mu and E to 1e-10 relative.  Parity windows follow DESIGN.md section 4 (collapse regime, R#27)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_1610_05329_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_1 = 1e-12
+TOL_100 = 1e-10
+TOL_OBS = 1e-10
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_1610_05329_b200 import binding
+    binding.lib()
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def pair(gpu, oracle, shape, d, dt, trap, g, gdd, mode):
+    return (gpu.Dgpe(*shape, *d, dt, *trap, g, gdd, mode), oracle.Oracle(*shape, *d, dt, *trap, g, gdd, mode))
+
+
+# shapes span: one tile, ragged last tiles (line counts not multiples of 8), radix 3, several FFT passes,
+# nz = 2*odd, minimum size 4, non-cubic
+STAGE_SHAPES = [(4, 4, 4), (8, 8, 8), (6, 9, 12), (12, 18, 16), (27, 32, 6), (16, 24, 36), (64, 64, 64),
+                (48, 96, 128), (9, 4, 18)]
+
+
+@pytest.mark.parametrize("shape", STAGE_SHAPES)
+@pytest.mark.parametrize("mode", [0, 1])
+def test_stage_parity(gpu, oracle, shape, mode):
+    G, O = pair(gpu, oracle, shape, (0.3, 0.25, 0.2), 0.01, (1.0, 0.7, 1.3), 5.0, 3.0, mode)
+    psi = inputs.random_state(shape, 3) * 0.3
+    # (a) dipolar mean field
+    phi = G.dipolar(dev(psi)).cpu().numpy()
+    ref = O.dipolar(np.ascontiguousarray(psi.real ** 2 + psi.imag ** 2))
+    assert np.max(np.abs(phi - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref)))
+    # (a)+(b) nonlinear exponential
+    t, a = dev(psi), psi.copy()
+    G.nonlinear(t)
+    O.nonlinear(a)
+    assert np.max(np.abs(t.cpu().numpy() - a)) <= TOL_1
+    # (c) each sweep
+    for axis in range(3):
+        t, a = dev(psi), psi.copy()
+        G.sweep(t, axis)
+        O.sweep(a, axis)
+        out = t.cpu().numpy()
+        assert np.max(np.abs(out - a)) <= TOL_1, axis
+        # Dirichlet end nodes are written as exact zeros
+        sl = [slice(None)] * 3
+        for end in (0, -1):
+            sl[axis] = end
+            assert np.all(out[tuple(sl)] == 0)
+    # observables
+    t = dev(psi)
+    got = [G.norm(t), *G.rms(t), *G.energy_terms(t), G.chempot(t), G.energy(t)]
+    exp = [O.norm(psi), *O.rms(psi), *O.energy_terms(psi), O.chempot(psi), O.energy(psi)]
+    for x, y in zip(got, exp):
+        assert abs(x - y) <= TOL_OBS * max(1.0, abs(y))
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("dt", [0.5, 5.0, 40.0])
+def test_sweeps_with_large_r_need_the_long_lookback(gpu, oracle, mode, dt):
+    """r = dt/(4 d^2) up to 250: the chunk factors are O(1), so the inflow look-back spans many chunks."""
+    shape = (64, 48, 96)
+    G, O = pair(gpu, oracle, shape, (0.3, 0.25, 0.2), dt, (1.0, 1.0, 1.0), 0.0, 0.0, mode)
+    psi = inputs.random_state(shape, 5)
+    for axis in range(3):
+        t, a = dev(psi), psi.copy()
+        G.sweep(t, axis)
+        O.sweep(a, axis)
+        assert np.max(np.abs(t.cpu().numpy() - a)) <= 1e-12 * (1 + dt), axis
+
+
+def run_both(gpu, oracle, cfg, checkpoints, psi0=None):
+    """Step GPU and oracle side by side; at each checkpoint return (step, max|dpsi|, obs_gpu, obs_ref)."""
+    psi0 = inputs.initial_state(cfg) if psi0 is None else psi0
+    G, O = gpu.Dgpe(*cfg.create_args()), oracle.Oracle(*cfg.create_args())
+    t, a = dev(psi0), psi0.copy()
+    done, out = 0, []
+    for cp in checkpoints:
+        rc_g = G.step(t, cp - done)
+        rc_o = O.step(a, cp - done)
+        done = cp
+        assert rc_g == rc_o
+        err = float(np.max(np.abs(t.cpu().numpy() - a)))
+        og = [G.norm(t), G.chempot(t), G.energy(t), *G.rms(t)]
+        orf = [O.norm(a), O.chempot(a), O.energy(a), *O.rms(a)]
+        out.append((cp, err, og, orf))
+    return out, t, a
+
+
+def check_obs(og, orf):
+    for x, y in zip(og, orf):
+        assert abs(x - y) <= TOL_OBS * max(1.0, abs(y)), (og, orf)
+
+
+def test_c1_full_config_1_and_100_steps(gpu, oracle):
+    """BJ:configs[0], literally: 64^3 imaginary time, 100 steps with renormalisation each step."""
+    res, t, a = run_both(gpu, oracle, inputs.CONFIGS["C1"], [1, 10, 100])
+    for cp, err, og, orf in res:
+        assert err <= (TOL_1 if cp == 1 else TOL_100), (cp, err)
+        check_obs(og, orf)
+        assert abs(og[0] - 1.0) <= 1e-13          # imaginary time returns unit norm
+
+
+def test_c2_128cubed_1_and_20_steps(gpu, oracle):
+    """BJ:configs[1] on its full 128^3 grid (smooth window)."""
+    res, _, _ = run_both(gpu, oracle, inputs.CONFIGS["C2"], [1, 20])
+    for cp, err, og, orf in res:
+        assert err <= (TOL_1 if cp == 1 else TOL_100), (cp, err)
+        check_obs(og, orf)
+
+
+def test_c3_protocol_scaled_relax_then_quench_real_time(gpu, oracle):
+    """BJ:configs[2] protocol on a 48^3 box with the same spacings: imaginary-time relaxation with
+    g = 80, then real time after the quench to g = 64; norm conserved at every checkpoint."""
+    cfg = inputs.scaled(inputs.CONFIGS["C3"], (48, 48, 48))
+    res, t, a = run_both(gpu, oracle, cfg.relax, [1, 60])
+    for cp, err, og, orf in res:
+        assert err <= (TOL_1 if cp == 1 else TOL_100)
+        check_obs(og, orf)
+    # quench: continue each side from ITS OWN relaxed state (they agree to TOL_100)
+    G, O = gpu.Dgpe(*cfg.create_args()), oracle.Oracle(*cfg.create_args())
+    n0 = G.norm(t)
+    done = 0
+    for cp in (1, 10, 100):
+        G.step(t, cp - done)
+        O.step(a, cp - done)
+        done = cp
+        assert np.max(np.abs(t.cpu().numpy() - a)) <= 2 * TOL_100
+        assert abs(G.norm(t) - n0) <= 1e-12        # BJ:north_star check (4)
+        check_obs([G.chempot(t), G.energy(t), *G.rms(t)], [O.chempot(a), O.energy(a), *O.rms(a)])
+
+
+def test_c5_scaled_non_cubic_radix3_real_time(gpu, oracle):
+    """BJ:configs[4] on 96x96x48 (same spacings, radix-3 passes on every axis): seeded phase field,
+    real time, norm and energy tracked."""
+    cfg = inputs.scaled(inputs.CONFIGS["C5"], (96, 96, 48))
+    res, _, _ = run_both(gpu, oracle, cfg, [1, 10, 100])
+    for cp, err, og, orf in res:
+        assert err <= (TOL_1 if cp == 1 else TOL_100), (cp, err)
+        check_obs(og, orf)
+        assert abs(og[0] - 1.0) <= 1e-12
+
+
+def test_c4_physics_scaled_smooth_window_and_nonfinite_status(gpu, oracle):
+    """BJ:configs[3] physics on a 64^3 box: parity inside the smooth window (steps 1, 10), and both
+    sides must agree on the status of the literal long call (collapse regime, R#27: no clamp)."""
+    cfg = inputs.scaled(inputs.CONFIGS["C4"], (64, 64, 64))
+    res, t, a = run_both(gpu, oracle, cfg, [1, 10])
+    for cp, err, og, orf in res:
+        assert err <= (TOL_1 if cp == 1 else TOL_100), (cp, err)
+        check_obs(og, orf)
+    G, O = gpu.Dgpe(*cfg.create_args()), oracle.Oracle(*cfg.create_args())
+    rc_g, rc_o = G.step(t, 190), O.step(a, 190)
+    assert rc_g == rc_o
+    if rc_g == gpu.ERR_NONFINITE:
+        assert "norm" in gpu.last_error()
+
+
+def test_256cubed_single_real_time_step(gpu, oracle):
+    """BJ:configs[2] grid at full size (256^3, real-time handle), one step from the seeded Gaussian."""
+    cfg = inputs.CONFIGS["C3"]
+    psi0 = inputs.initial_state(cfg)
+    G, O = gpu.Dgpe(*cfg.create_args()), oracle.Oracle(*cfg.create_args())
+    t, a = dev(psi0), psi0.copy()
+    G.step(t, 1)
+    O.step(a, 1)
+    assert np.max(np.abs(t.cpu().numpy() - a)) <= TOL_1
+    assert abs(G.norm(t) - 1.0) <= 1e-12
+
+
+def test_edge_cases(gpu, oracle):
+    G, O = pair(gpu, oracle, (8, 12, 4), (0.5, 0.4, 0.3), 0.01, (1.0, 1.0, 1.0), 1.0, 1.0, 0)
+    psi = inputs.random_state((8, 12, 4), 9)
+    t = dev(psi)
+    before = t.clone()
+    assert G.step(t, 0) == gpu.OK                   # empty call: no-op
+    assert torch.equal(t, before)
+    z = torch.zeros((8, 12, 4), dtype=torch.complex128, device="cuda")
+    assert G.step(z, 1) == gpu.ERR_NONFINITE        # zero state: norm 0 -> same status as the oracle
+    a = np.zeros((8, 12, 4), dtype=np.complex128)
+    assert O.step(a, 1) == oracle.ERR_NONFINITE
+    with pytest.raises(TypeError):
+        G.step(t.to(torch.complex64), 1)
+    with pytest.raises(gpu.DgpeError):
+        G.sweep(t, 3)
+    # un-normalised, non-zero faces on input: the step ignores the faces in the sweeps (R#8)
+    psi2 = inputs.random_state((8, 12, 4), 10, zero_faces=False) * 3.0
+    t, a = dev(psi2), psi2.copy()
+    assert G.step(t, 2) == O.step(a, 2) == 0
+    assert np.max(np.abs(t.cpu().numpy() - a)) <= TOL_1
+
+
+def test_step_host_matches_device_path(gpu):
+    cfg = inputs.CONFIGS["C1"]
+    psi0 = inputs.initial_state(cfg)
+    G = gpu.Dgpe(*cfg.create_args())
+    t = dev(psi0)
+    G.step(t, 3)
+    hp = torch.from_numpy(psi0.copy()).pin_memory()
+    assert G.step_host(hp, 3) == gpu.OK
+    assert torch.equal(hp, t.cpu())                 # same kernels, deterministic reductions: bit-identical
+
+
+def test_bitwise_repeatable(gpu):
+    cfg = inputs.CONFIGS["C1"]
+    psi0 = inputs.initial_state(cfg)
+    G = gpu.Dgpe(*cfg.create_args())
+    a, b = dev(psi0), dev(psi0)
+    G.step(a, 5)
+    G.step(b, 5)
+    assert torch.equal(a, b)
+
+
+# ------------------------------------------------------------------------------------------------
+# full BASELINE sizes, in the launch configuration bench.py times (512^3, C4 handle)
+# ------------------------------------------------------------------------------------------------
+
+@pytest.fixture(scope="module")
+def c4(gpu):
+    cfg = inputs.CONFIGS["C4"]
+    return cfg, gpu.Dgpe(*cfg.create_args())
+
+
+def test_fullsize_dipolar_plane_wave_closed_form(gpu, c4):
+    """n = 1 + sum a_m cos(q_m.r + p_m), q_m grid wave vectors  =>  Phi = sum Udd~(q_m) a_m cos(...)
+    exactly (pin P4), at 512^3 through the production kernels K1-K5."""
+    cfg, G = c4
+    nx, ny, nz = cfg.shape
+    L = [n * d for n, d in zip(cfg.shape, cfg.d)]
+    x, y, z = [torch.from_numpy(inputs.coords(n, d)).cuda() for n, d in zip(cfg.shape, cfg.d)]
+    waves = [((3, 0, 0), 0.11, 0.3), ((0, 0, 5), 0.07, 1.1), ((2, -7, 1), 0.05, 2.0), ((-100, 31, 255), 0.02, 0.5),
+             ((0, 256, 0), 0.01, 0.0)]
+    dens = torch.ones(cfg.shape, dtype=torch.float64, device="cuda")
+    phi_ref = torch.zeros_like(dens)
+    for m, amp, ph in waves:
+        q = [2 * np.pi * mi / Li for mi, Li in zip(m, L)]
+        udd = (4 * np.pi / 3) * (3 * q[2] ** 2 / (q[0] ** 2 + q[1] ** 2 + q[2] ** 2) - 1)
+        w = torch.cos(q[0] * x[:, None, None] + q[1] * y[None, :, None] + q[2] * z[None, None, :] + ph)
+        dens += amp * w
+        phi_ref += udd * amp * w
+        del w
+    psi = torch.sqrt(dens).to(torch.complex128)
+    phi = G.dipolar(psi)
+    assert float((phi - phi_ref).abs().max()) <= 1e-12
+    del phi, phi_ref, dens, psi
+    torch.cuda.empty_cache()
+
+
+def test_fullsize_sweeps_sampled_lines(gpu, oracle, c4):
+    """At 512^3 each sweep is compared, on 64 sampled lines per axis, with the oracle's solve of the
+    same lines (the oracle sweeps a 512 x 8 x 8 array holding the sampled lines)."""
+    cfg, G = c4
+    n = 512
+    gen = torch.Generator(device="cuda").manual_seed(11)
+    psi = torch.randn(cfg.shape, dtype=torch.float64, device="cuda", generator=gen).to(torch.complex128)
+    psi += 1j * torch.randn(cfg.shape, dtype=torch.float64, device="cuda", generator=gen)
+    rng = np.random.default_rng(12)
+    for axis in range(3):
+        out = psi.clone()
+        G.sweep(out, axis)
+        ia, ib = rng.integers(0, n, 64), rng.integers(0, n, 64)
+        ia[:4], ib[:4] = [0, 0, n - 1, n - 1], [0, n - 1, 0, n - 1]        # include edge lines
+        sel = (torch.from_numpy(ia).cuda(), torch.from_numpy(ib).cuda())
+        if axis == 0:
+            lin, lout = psi[:, sel[0], sel[1]], out[:, sel[0], sel[1]]             # (512, 64)
+        elif axis == 1:
+            lin, lout = psi[sel[0], :, sel[1]].T, out[sel[0], :, sel[1]].T
+        else:
+            lin, lout = psi[sel[0], sel[1], :].T, out[sel[0], sel[1], :].T
+        d = cfg.d[axis]
+        O = oracle.Oracle(n, 8, 8, d, 1.0, 1.0, cfg.dt, 1, 1, 1, 0.0, 0.0, cfg.mode)
+        a = np.ascontiguousarray(lin.cpu().numpy().reshape(n, 8, 8))
+        O.sweep(a, 0)
+        assert np.max(np.abs(lout.cpu().numpy().reshape(n, 8, 8) - a)) <= TOL_1, axis
+        del out
+    del psi
+    torch.cuda.empty_cache()
+
+
+def test_fullsize_step_properties(gpu, c4):
+    """Literal C4 at 512^3 (the configuration bench.py times): one imaginary-time step returns unit
+    norm; with g = gdd = 0 the harmonic ground state is a fixed point of the normalised step up to the
+    O(dt, dx^2) splitting error, and mu -> (gamma+nu+lambda)/2 (BJ:north_star check 3)."""
+    cfg, G = c4
+    psi = dev(inputs.initial_state(cfg))
+    assert G.step(psi, 1) == gpu.OK
+    assert abs(G.norm(psi) - 1.0) <= 1e-13
+    assert bool(torch.isfinite(torch.view_as_real(psi)).all())
+    for face in (psi[0], psi[-1], psi[:, 0], psi[:, -1], psi[:, :, 0], psi[:, :, -1]):
+        assert float(face.abs().max()) == 0.0
+    del psi
+    torch.cuda.empty_cache()
+    free = inputs.Config("C4-free", cfg.shape, cfg.d, cfg.dt, cfg.trap, 0.0, 0.0, 0, 1, 4, cfg.gauss, noise=0.0)
+    G0 = gpu.Dgpe(*free.create_args())
+    p0 = dev(inputs.initial_state(free))
+    p1 = p0.clone()
+    G0.step(p1, 20)
+    assert float((p1 - p0).abs().max()) <= 2e-3 * float(p0.abs().max())
+    mu = G0.chempot(p1)
+    assert abs(mu - 0.5 * sum(cfg.trap)) <= 0.5 * sum(w * w * d * d / 16 for w, d in zip(cfg.trap, cfg.d)) + 5e-3
+    assert abs(mu - G0.energy(p1)) <= 1e-12        # no interaction: mu == E
