@@ -1,0 +1,285 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the full SSCN step (BASELINE.json metric: fp64 SSCN steps/s and grid-point
+updates/s at 512^3 on one B200; HBM GB/s vs peak).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--impl reference]
+
+One "step" = one pass of the whole hot path (kernels K1..K8) over the psi of the
+workload.  N = 1 times BASELINE.json's headline configuration C4 (512^3, imaginary time).  N > 1
+(torchrun, one rank per GPU) runs N independent replicas -- the path does not shard without all-to-all
+transposes -- and reports all ranks' steps over the slowest rank's time.
+Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle instead (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "sscn_steps_per_s"
+UNIT = "steps/s"
+# the oracle is ~160 s per 512^3 step on one core, so its legs run a bounded sample of the workload:
+# the same physics (spacings, dt, trap, g, gdd, seeded state recipe) on a smaller centred box
+CPU_SAMPLE_BASELINE = (256, 256, 128)    # cpu_baseline leg: one step, ~10 s
+CPU_SAMPLE_REFERENCE = (128, 128, 128)   # --impl reference: every step, ~2 s each
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C4")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(cfg):
+    nx, ny, nz = cfg.shape
+    mode = "imaginary-time" if cfg.mode == 0 else "real-time"
+    return (f"{cfg.name}: {mode} dipolar GPE {nx}x{ny}x{nz} fp64 complex, dx={cfg.d[0]} dt={cfg.dt} "
+            f"trap={cfg.trap} g={cfg.g} gdd={cfg.gdd} (BASELINE.json configs[{int(cfg.name[1]) - 1}])")
+
+
+def load_peaks():
+    """Measured roofline denominators (driver-written); else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc, self.thread = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            p = [x.strip() for x in r.split(",")]
+            if len(p) < 7:
+                continue
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1])); pw.append(float(p[2]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, p[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+# the CPU oracle, timed as it stands (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------------
+def oracle_time(cfg, sample_shape, steps, warmup=0):
+    """Seconds per oracle step on a `sample_shape` box with cfg's physics; returns (s/step, npoints)."""
+    from oracle import binding as ob
+    from paper_1610_05329_b200 import inputs
+    sub = inputs.scaled(cfg, sample_shape)
+    psi = inputs.initial_state(sub)
+    O = ob.Oracle(*sub.create_args())
+    if warmup:
+        O.step(psi, warmup)
+    t0 = time.perf_counter()
+    O.step(psi, steps)
+    dt = time.perf_counter() - t0
+    return dt / steps, sub.npoints
+
+
+def cpu_baseline(cfg, sample_shape, steps=1):
+    s_per_step, npts = oracle_time(cfg, sample_shape, steps)
+    pts_per_s = npts / s_per_step
+    return {"value": pts_per_s / cfg.npoints, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "grid_pt_updates_per_s": pts_per_s,
+            "sample": (f"{steps} oracle step(s) of {cfg.name}'s physics on a {'x'.join(map(str, sample_shape))} box "
+                       f"({npts / cfg.npoints:.4f} of the points), {s_per_step:.2f} s/step on 1 core of "
+                       f"{os.cpu_count()}; value = sample grid-pt updates/s / {cfg.npoints} points")}
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    s_per_step, npts = oracle_time(cfg, CPU_SAMPLE_REFERENCE, args.steps, args.warmup)
+    pts_per_s = npts / s_per_step
+    value = pts_per_s / cfg.npoints
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / value, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "grid_pt_updates_per_s": pts_per_s,
+        "config": {"workload": workload_name(cfg), "sample_box": list(CPU_SAMPLE_REFERENCE)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": (f"each step = one oracle step of {cfg.name}'s physics on a "
+                                    f"{'x'.join(map(str, CPU_SAMPLE_REFERENCE))} box, {s_per_step:.2f} s/step, scaled by "
+                                    f"points to the {cfg.npoints}-point workload")},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA path
+# ------------------------------------------------------------------------------------------------
+def ncu_traffic(kernel_name):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, if one is recorded
+    in profiles/traffic.json ({kernel name: bytes}); else None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(kernel_name)
+    except Exception:
+        return None
+
+
+def run_b200(args, cfg):
+    import torch
+    from paper_1610_05329_b200 import binding, inputs, replicas
+    from dataclasses import replace
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    rank, local_rank, world = replicas.init()
+    torch.cuda.set_device(local_rank)
+    K, W = args.steps, max(args.warmup, 3)
+    mycfg = replace(cfg, seed=replicas.replica_seed(cfg.seed, rank))       # each replica: its own seeded state
+
+    G = binding.Dgpe(*mycfg.create_args())
+    psi_host = torch.from_numpy(inputs.initial_state(mycfg)).pin_memory()
+    psi0 = psi_host.cuda()
+    psi = psi0.clone()
+
+    # ---- device-resident timing: inputs in HBM when the timed region starts ----
+    G.step(psi, W)
+    psi.copy_(psi0)
+    torch.cuda.synchronize()
+    replicas.barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    status = G.step(psi, K)
+    e1.record()
+    torch.cuda.synchronize()
+    replicas.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    sec_local = e0.elapsed_time(e1) * 1e-3
+    value, sec = replicas.aggregate_throughput(K, sec_local)
+    finite = bool(torch.isfinite(torch.view_as_real(psi)).all())
+
+    # ---- per-kernel durations, CUDA events on the handle's stream (dgpe_step_profile) ----
+    psi.copy_(psi0)
+    G.step_profile(psi, 2)
+    psi.copy_(psi0)
+    prof = G.step_profile(psi, min(K, 8))
+    peak, peak_src = load_peaks()
+    kernels = [{"name": n, "bytes": b, "ms": ms, "GBps": b / ms * 1e-6} for n, b, ms in prof]
+    top = max(kernels, key=lambda k: k["ms"])
+    step_ms = sec_local / K * 1e3
+    roofline = {"bound": "hbm", "kernel": top["name"], "achieved": top["GBps"], "peak": peak, "unit": "GB/s",
+                "frac": top["GBps"] / peak, "traffic": ncu_traffic(top["name"]), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": top["bytes"], "kernel_ms": top["ms"],
+                "share_of_step": top["ms"] / sum(k["ms"] for k in kernels)}
+    step_gbps = G.bytes_per_step / step_ms * 1e-6
+    whole = {"algorithmic_bytes_per_step": G.bytes_per_step, "achieved": step_gbps, "frac": step_gbps / peak,
+             "unit": "GB/s", "model": "M1 = 144N + 8S (DESIGN.md section 7)"}
+
+    # ---- end to end through the C-ABI with HOST buffers (dgpe_step_host) ----
+    e2e = None
+    if not args.no_e2e:
+        work = psi_host.clone().pin_memory()
+        G.step_host(work, 1)                      # allocates the staging buffer, warms the copies
+        work.copy_(psi_host)
+        torch.cuda.synchronize()
+        replicas.barrier()
+        t0 = time.perf_counter()
+        G.step_host(work, K)                      # H2D + K steps + D2H, returns after the stream is idle
+        e2e_local = time.perf_counter() - t0
+        replicas.barrier()
+        e2e_value, _ = replicas.aggregate_throughput(K, e2e_local)
+        nbytes = work.numel() * 16
+        e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes / K, "d2h_bytes_per_step": nbytes / K,
+               "call": f"dgpe_step_host(psi_pinned, {K}): one H2D of psi ({nbytes} B), {K} steps, one D2H; bytes per "
+                       f"step = bytes per call / {K}", "ms_per_call": e2e_local * 1e3}
+        del work
+
+    if rank != 0:
+        replicas.shutdown()
+        return
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": sec / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "grid_pt_updates_per_s": value * cfg.npoints,
+        "config": {"workload": workload_name(cfg), "parallelism": f"replicas x{world} (no sharding, no collectives)",
+                   "l2": "inputs larger than L2: psi %.2f GB + half-spectrum %.2f GB vs 126 MB" %
+                         (cfg.npoints * 16e-9, cfg.shape[0] * cfg.shape[1] * (cfg.shape[2] // 2 + 1) * 16e-9),
+                   "status": int(status), "finite": finite,
+                   "note": "literal C4 is in the dipolar-collapse regime: NaN from step ~19 (DESIGN.md section 4); "
+                           "timing is data-independent"},
+        "clocks": clocks, "gpu_launches": K * G.launches_per_step + (3 if cfg.mode == 0 else 1),
+        "roofline": roofline, "step_roofline": whole, "kernels": kernels,
+    }
+    if e2e is not None:
+        line["e2e"] = e2e
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(cfg, CPU_SAMPLE_BASELINE)
+    print(json.dumps(line), flush=True)
+    replicas.shutdown()
+
+
+def main():
+    args = parse()
+    from paper_1610_05329_b200 import inputs
+    cfg = inputs.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_b200(args, cfg)
+
+
+if __name__ == "__main__":
+    main()
