@@ -1,0 +1,190 @@
+// ctfft.cuh -- compile-time-planned Stockham passes whose butterflies live in registers, used by the
+// specialised kernels in xyfft.cuh (strided axes x, y) and zline.cuh (contiguous axis z).
+//
+// Same mathematics as fft.cuh (P:L130 FFT-friendly sizes 2^a 3^b; BJ:north_star "mixed-radix
+// (2^a 3^b) shared-memory Stockham FFT passes per axis"): pass p with radix R and Ns = product of the
+// radices before it computes, for every butterfly j in [0, N/R), k = j mod Ns,
+//     v_q = in[j + q N/R] w_N^{q k N/(Ns R)},    out[(j div Ns) Ns R + k + s Ns] = sum_q v_q w_R^{q s}.
+// Here N and the radix sequence are template constants, so every index folds at compile time and a
+// thread keeps its butterflies in registers between the read side and the write side of a pass.
+// The radix sequence is 8.., 4, 2, 3.. (REV = false) or its reverse (REV = true).  With the reversed
+// sequence the first pass of a transform reads exactly the elements the last pass of a forward-order
+// transform produced in the same thread, so a forward and an inverse transform chain in registers
+// (K3: FFT_x, multiply by Udd~(k), IFFT_x -- BJ:north_star).
+#pragma once
+#include "fft.cuh"
+
+namespace dgpe {
+namespace ct {
+
+__host__ __device__ constexpr int pick(int m) { return (m % 8 == 0) ? 8 : (m % 4 == 0) ? 4 : (m % 2 == 0) ? 2 : 3; }
+__host__ __device__ constexpr int npass(int n)
+{
+    int c = 0;
+    while (n > 1) { n /= pick(n); ++c; }
+    return c;
+}
+__host__ __device__ constexpr int radix_fwd(int n, int p)
+{
+    for (int i = 0; i < p; ++i) n /= pick(n);
+    return pick(n);
+}
+__host__ __device__ constexpr int radix_at(int n, int p, bool rev) { return radix_fwd(n, rev ? npass(n) - 1 - p : p); }
+__host__ __device__ constexpr int ns_at(int n, int p, bool rev)
+{
+    int ns = 1;
+    for (int i = 0; i < p; ++i) ns *= radix_at(n, i, rev);
+    return ns;
+}
+__host__ __device__ constexpr int rmax(int n)
+{
+    int r = 1;
+    while (n > 1) { int q = pick(n); if (q > r) r = q; n /= q; }
+    return r;
+}
+__host__ __device__ constexpr bool smooth(int n)
+{
+    if (n < 1) return false;
+    while (n % 2 == 0) n /= 2;
+    while (n % 3 == 0) n /= 3;
+    return n == 1;
+}
+
+}  // namespace ct
+
+// Pass P of an N-point transform for a team of NBF butterfly slots (slot b handles butterflies
+// b, b + NBF, ...).  load -> (barrier, if the passes run in place) -> bfly -> scatter.
+template <int N, int P, bool INV, bool REV, int NBF>
+struct CtPass {
+    static constexpr int R = ct::radix_at(N, P, REV);
+    static constexpr int Ns = ct::ns_at(N, P, REV);
+    static constexpr int NBUT = N / R;
+    static constexpr int NB = (NBUT + NBF - 1) / NBF;
+    static constexpr bool EXACT = (NBUT % NBF) == 0;
+    static constexpr int TWSTEP = N / (Ns * R);
+    static constexpr int NPASS = ct::npass(N);
+    static constexpr bool LAST = (P == NPASS - 1);
+
+    cplx v[NB][R];
+
+    // v_q = f(j + q N/R) for this slot's butterflies, then the twiddles (tw[m] = exp(-2 pi i m/N))
+    template <class F>
+    __device__ __forceinline__ void load(int b, const cplx* __restrict__ tw, F&& f)
+    {
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            const int j = b + u * NBF;
+            if (EXACT || j < NBUT) {
+#pragma unroll
+                for (int q = 0; q < R; ++q) v[u][q] = f(j + q * NBUT);
+                if (Ns > 1) {
+                    const int k = j % Ns;
+#pragma unroll
+                    for (int q = 1; q < R; ++q) {
+                        cplx w = __ldg(&tw[q * k * TWSTEP]);
+                        if (INV) w.y = -w.y;
+                        v[u][q] = cmul(v[u][q], w);
+                    }
+                }
+            }
+        }
+    }
+
+    __device__ __forceinline__ void bfly(int b)
+    {
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            const int j = b + u * NBF;
+            if (EXACT || j < NBUT) Butterfly<R, INV>::run(v[u]);
+        }
+    }
+
+    // f(output index, value) for every output of this slot; for_each may also rewrite v in place
+    template <class F>
+    __device__ __forceinline__ void scatter(int b, F&& f)
+    {
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            const int j = b + u * NBF;
+            if (EXACT || j < NBUT) {
+                const int k = j % Ns;
+                const int base = (j / Ns) * Ns * R + k;
+#pragma unroll
+                for (int s = 0; s < R; ++s) f(base + s * Ns, v[u][s]);
+            }
+        }
+    }
+    template <class F>
+    __device__ __forceinline__ void modify(int b, F&& f)     // v <- f(output index, v)
+    {
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            const int j = b + u * NBF;
+            if (EXACT || j < NBUT) {
+                const int k = j % Ns;
+                const int base = (j / Ns) * Ns * R + k;
+#pragma unroll
+                for (int s = 0; s < R; ++s) v[u][s] = f(base + s * Ns, v[u][s]);
+            }
+        }
+    }
+};
+
+// Barrier between the passes of one team: the whole CTA (strided-axis tiles) or one warp (z lines).
+struct SyncCta { static __device__ __forceinline__ void sync() { __syncthreads(); } };
+struct SyncWarp { static __device__ __forceinline__ void sync() { __syncwarp(); } };
+
+// Passes P .. PEND-1 of an N-point transform, in place in a shared-memory column: element idx of the
+// column lives at col[Pos::at(idx)].  Pass P takes its inputs from `first(idx)` if FROM_F (else from
+// the column).  The final pass of the transform (P = NPASS-1) hands its outputs to `last(idx, value)`;
+// every other pass writes the column and ends with a team barrier.
+// `on` = this thread owns butterfly slot b (threads that do not still take part in the barriers).
+// When FROM_F is false the caller must have synchronised the team after the column was written; when
+// it is true the column must be free to overwrite.
+template <int N, bool INV, bool REV, int NBF, class Sync, class Pos, int P, int PEND, bool FROM_F, class FFirst,
+          class FLast>
+__device__ __forceinline__ void ct_fft_range(cplx* col, int b, bool on, const cplx* __restrict__ tw, FFirst&& first,
+                                             FLast&& last)
+{
+    if constexpr (P < PEND) {
+        using Pass = CtPass<N, P, INV, REV, NBF>;
+        Pass pass;
+        if (on) {
+            if constexpr (FROM_F) pass.load(b, tw, first);
+            else pass.load(b, tw, [&](int idx) { return col[Pos::at(idx)]; });
+        }
+        if constexpr (!FROM_F) Sync::sync();          // every read of this pass precedes its writes
+        if (on) pass.bfly(b);
+        if constexpr (Pass::LAST) {
+            if (on) pass.scatter(b, last);
+        } else {
+            if (on) pass.scatter(b, [&](int idx, cplx val) { col[Pos::at(idx)] = val; });
+            Sync::sync();
+            ct_fft_range<N, INV, REV, NBF, Sync, Pos, P + 1, PEND, false>(col, b, on, tw, first, last);
+        }
+    }
+}
+
+// ---- streaming global accesses (every array of the step is far larger than L2) ----
+__device__ __forceinline__ cplx ld_stream(const cplx* p)
+{
+    cplx v;
+    asm volatile("ld.global.cs.v2.f64 {%0, %1}, [%2];\n" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st_stream(cplx* p, cplx v)
+{
+    asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};\n" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+
+// ---- cp.async (LDGSTS): 16 bytes per thread straight into shared memory, L2-only caching ----
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int NKEEP>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(NKEEP) : "memory"); }
+
+}  // namespace dgpe

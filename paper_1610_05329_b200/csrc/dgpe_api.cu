@@ -8,6 +8,7 @@
 #include <complex>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -16,6 +17,8 @@
 #include "observe.cuh"
 #include "spectral.cuh"
 #include "sweep.cuh"
+#include "xyfft.cuh"
+#include "xysweep.cuh"
 
 using namespace dgpe;
 
@@ -62,6 +65,8 @@ struct dgpe_handle {
     double dx, dy, dz, dt, gamma, nu, lambda, g, gdd;
     long long N;
     cudaStream_t stream = nullptr;
+    int num_sms = 148;
+    bool force_generic = false;      // DGPE_GENERIC=1: runtime-plan kernels only (A/B checks)
 
     cplx* spec = nullptr;                       // [nx][ny][nzh]
     FftPlan plan_x{}, plan_y{}, plan_zh{};      // transform lengths nx, ny, nz/2
@@ -168,7 +173,7 @@ static int build_sweep(dgpe_handle* h, AxisSweep* S, int n, std::complex<double>
     typedef std::complex<double> C;
     S->n = n;
     S->r = r;
-    S->Lc = 16;
+    S->Lc = (n <= 514 && !h->force_generic) ? 8 : 16;
     const int nun = n - 2;
     S->G = (nun + S->Lc - 1) / S->Lc;
     std::vector<C> inv(n, C(0)), cc(n, C(0)), F(n, C(0)), Gm(n, C(0)), A(S->G, C(0)), B(S->G, C(0));
@@ -238,6 +243,13 @@ static int init_handle(dgpe_handle* h)
     int dev_count = 0;
     CU(cudaGetDeviceCount(&dev_count));
     if (dev_count < 1) return fail(DGPE_ERR_CUDA, "no CUDA device");
+    {
+        int dev = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev));
+        const char* e = getenv("DGPE_GENERIC");
+        h->force_generic = e && e[0] == '1';
+    }
 
     if ((rc = make_plan(h, nx, &h->plan_x, &h->tw_x))) return rc;
     if ((rc = make_plan(h, ny, &h->plan_y, &h->tw_y))) return rc;
@@ -393,40 +405,106 @@ static int check_launch(const char* what)
     return DGPE_OK;
 }
 
-// K1..K4: spec <- Udd~(k)/N * FFT(s2 |psi|^2), transformed back along x and y
-static int launch_dipolar_spectrum(dgpe_handle* h, const cplx* psi)
+// ---- K1 ----
+static int launch_k1(dgpe_handle* h, const cplx* psi)
 {
-    const int nx = h->nx, ny = h->ny, nz = h->nz, nzh = h->nzh, M = nz / 2;
-    const int nlines = nx * ny;
-    int rc;
+    const int nlines = h->nx * h->ny, M = h->nz / 2;
     k_dens_r2c<<<(nlines + 7) / 8, threads_for(h->plan_zh.nbf), sizeof(cplx) * TILE_COLS * (size_t)M, h->stream>>>(
-        psi, h->spec, nlines, nz, h->plan_zh, h->tw_split, h->scal);
-    if ((rc = check_launch("k_dens_r2c"))) return rc;
+        psi, h->spec, nlines, h->nz, h->plan_zh, h->tw_split, h->scal);
+    return check_launch("k_dens_r2c");
+}
 
+// ---- K2 / K4 (axis 1) and K3 (axis 0): pipelined compile-time kernels when the length is one of the
+// specialised sizes, else the generic runtime-plan kernels ----
+template <int N, int KIND>
+static int launch_fft_xy_n(dgpe_handle* h, const LineMap& map, int nbatch, const cplx* tw)
+{
+    const size_t smem = (size_t)N * TILE_COLS * sizeof(cplx);
+    auto kern = k_fft_xy<N, KIND>;
+    static bool ready = false;           // per instantiation (one device per process)
+    if (!ready) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ready = true;
+    }
+    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 1.0 / (double)h->N};
+    dim3 grid((map.ncols + TILE_COLS - 1) / TILE_COLS, nbatch);
+    kern<<<grid, xy_threads<N>(), smem, h->stream>>>(h->spec, map, tw, U);
+    return check_launch("k_fft_xy");
+}
+
+template <int KIND>
+static int launch_fft_xy(dgpe_handle* h, int n, const LineMap& map, int nbatch, const cplx* tw, bool* handled)
+{
+    *handled = true;
+    switch (n) {
+        case 8: return launch_fft_xy_n<8, KIND>(h, map, nbatch, tw);
+        case 16: return launch_fft_xy_n<16, KIND>(h, map, nbatch, tw);
+        case 32: return launch_fft_xy_n<32, KIND>(h, map, nbatch, tw);
+        case 48: return launch_fft_xy_n<48, KIND>(h, map, nbatch, tw);
+        case 64: return launch_fft_xy_n<64, KIND>(h, map, nbatch, tw);
+        case 96: return launch_fft_xy_n<96, KIND>(h, map, nbatch, tw);
+        case 128: return launch_fft_xy_n<128, KIND>(h, map, nbatch, tw);
+        case 192: return launch_fft_xy_n<192, KIND>(h, map, nbatch, tw);
+        case 256: return launch_fft_xy_n<256, KIND>(h, map, nbatch, tw);
+        case 384: return launch_fft_xy_n<384, KIND>(h, map, nbatch, tw);
+        case 512: return launch_fft_xy_n<512, KIND>(h, map, nbatch, tw);
+        case 768: return launch_fft_xy_n<768, KIND>(h, map, nbatch, tw);
+        case 1024: return launch_fft_xy_n<1024, KIND>(h, map, nbatch, tw);
+        default: *handled = false; return DGPE_OK;
+    }
+}
+
+static int launch_fft_y(dgpe_handle* h, bool inverse)
+{
+    const int nx = h->nx, ny = h->ny, nzh = h->nzh;
     LineMap my{ny, nzh, (long long)ny * nzh, 1, nzh};
+    if (!h->force_generic) {
+        bool handled = false;
+        int rc = inverse ? launch_fft_xy<FFT_INV>(h, ny, my, nx, h->tw_y, &handled)
+                         : launch_fft_xy<FFT_FWD>(h, ny, my, nx, h->tw_y, &handled);
+        if (rc || handled) return rc;
+    }
     dim3 gy((nzh + 7) / 8, nx);
-    const int ty = threads_for(h->plan_y.nbf), tx = threads_for(h->plan_x.nbf);
-    const size_t smy = sizeof(cplx) * TILE_COLS * (size_t)ny, smx = sizeof(cplx) * TILE_COLS * (size_t)nx;
-    if (ty <= 512)
-        k_fft_lines<false, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
-    else
-        k_fft_lines<false, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
-    if ((rc = check_launch("k_fft_lines<fwd,y>"))) return rc;
+    const int ty = threads_for(h->plan_y.nbf);
+    const size_t smy = sizeof(cplx) * TILE_COLS * (size_t)ny;
+    if (inverse) {
+        if (ty <= 512) k_fft_lines<true, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+        else k_fft_lines<true, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+    } else {
+        if (ty <= 512) k_fft_lines<false, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+        else k_fft_lines<false, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+    }
+    return check_launch("k_fft_lines<y>");
+}
 
+static int launch_fft_x_udd(dgpe_handle* h)
+{
+    const int nx = h->nx, ny = h->ny, nzh = h->nzh;
     LineMap mx{nx, ny * nzh, 0, 1, (long long)ny * nzh};
+    if (!h->force_generic) {
+        bool handled = false;
+        int rc = launch_fft_xy<FFT_X_UDD>(h, nx, mx, 1, h->tw_x, &handled);
+        if (rc || handled) return rc;
+    }
+    const int tx = threads_for(h->plan_x.nbf);
+    const size_t smx = sizeof(cplx) * TILE_COLS * (size_t)nx;
     if (tx <= 512)
         k_fft_x_udd<512><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
                                                                      1.0 / (double)h->N);
     else
         k_fft_x_udd<1024><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
                                                                       1.0 / (double)h->N);
-    if ((rc = check_launch("k_fft_x_udd"))) return rc;
+    return check_launch("k_fft_x_udd");
+}
 
-    if (ty <= 512)
-        k_fft_lines<true, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
-    else
-        k_fft_lines<true, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
-    return check_launch("k_fft_lines<inv,y>");
+// K1..K4: spec <- Udd~(k)/N * FFT(s2 |psi|^2), transformed back along x and y
+static int launch_dipolar_spectrum(dgpe_handle* h, const cplx* psi)
+{
+    int rc;
+    if ((rc = launch_k1(h, psi))) return rc;
+    if ((rc = launch_fft_y(h, false))) return rc;
+    if ((rc = launch_fft_x_udd(h))) return rc;
+    return launch_fft_y(h, true);
 }
 
 // K5 in one of its modes
@@ -465,6 +543,13 @@ static int launch_sweep_t(dgpe_handle* h, cplx* psi, int axis, bool fold)
     F.dV = h->dx * h->dy * h->dz;
     F.partials = h->partials; F.ticket = h->ticket; F.scal = h->scal;
     const int thr = threads_for(S.G);
+    if (axis < 2 && !h->force_generic && S.G <= 64 && (S.Lc == 8 || S.Lc == 16)) {
+        LineMap m = axis == 0 ? LineMap{nx, ny * nz, 0, 1, (long long)ny * nz} : LineMap{ny, nz, (long long)ny * nz, 1, nz};
+        dim3 grid((m.ncols + TILE_COLS - 1) / TILE_COLS, axis == 0 ? 1 : nx);
+        if (S.Lc == 8) k_sweep_xy<CT, 8, 512, 2><<<grid, thr, 0, h->stream>>>(psi, m, T, F);
+        else k_sweep_xy<CT, 16, 512, 1><<<grid, thr, 0, h->stream>>>(psi, m, T, F);
+        return check_launch("k_sweep_xy");
+    }
     if (axis == 0) {
         LineMap m{nx, ny * nz, 0, 1, (long long)ny * nz};
         k_sweep<CT, false><<<(ny * nz + 7) / 8, thr, sweep_smem(nx, S.G, false), h->stream>>>(psi, m, T, F);
@@ -501,38 +586,13 @@ static int one_step(dgpe_handle* h, cplx* psi, Mark mark)
     const int nx = h->nx, ny = h->ny, nz = h->nz, nzh = h->nzh, M = nz / 2;
     const int nlines = nx * ny;
     int rc;
-    // K1
-    k_dens_r2c<<<(nlines + 7) / 8, threads_for(h->plan_zh.nbf), sizeof(cplx) * TILE_COLS * (size_t)M, h->stream>>>(
-        psi, h->spec, nlines, nz, h->plan_zh, h->tw_split, h->scal);
-    if ((rc = check_launch("k_dens_r2c"))) return rc;
+    if ((rc = launch_k1(h, psi))) return rc;
     mark(0);
-    // K2
-    LineMap my{ny, nzh, (long long)ny * nzh, 1, nzh};
-    dim3 gy((nzh + 7) / 8, nx);
-    const int ty = threads_for(h->plan_y.nbf), tx = threads_for(h->plan_x.nbf);
-    const size_t smy = sizeof(cplx) * TILE_COLS * (size_t)ny, smx = sizeof(cplx) * TILE_COLS * (size_t)nx;
-    if (ty <= 512)
-        k_fft_lines<false, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
-    else
-        k_fft_lines<false, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
-    if ((rc = check_launch("k_fft_lines<fwd,y>"))) return rc;
+    if ((rc = launch_fft_y(h, false))) return rc;
     mark(1);
-    // K3
-    LineMap mx{nx, ny * nzh, 0, 1, (long long)ny * nzh};
-    if (tx <= 512)
-        k_fft_x_udd<512><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
-                                                                     1.0 / (double)h->N);
-    else
-        k_fft_x_udd<1024><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
-                                                                      1.0 / (double)h->N);
-    if ((rc = check_launch("k_fft_x_udd"))) return rc;
+    if ((rc = launch_fft_x_udd(h))) return rc;
     mark(2);
-    // K4
-    if (ty <= 512)
-        k_fft_lines<true, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
-    else
-        k_fft_lines<true, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
-    if ((rc = check_launch("k_fft_lines<inv,y>"))) return rc;
+    if ((rc = launch_fft_y(h, true))) return rc;
     mark(3);
     // K5
     if ((rc = launch_c2r(h, psi, imag ? 0 : 1, nullptr))) return rc;
