@@ -19,6 +19,7 @@
 #include "sweep.cuh"
 #include "xyfft.cuh"
 #include "xysweep.cuh"
+#include "zline.cuh"
 
 using namespace dgpe;
 
@@ -67,6 +68,7 @@ struct dgpe_handle {
     cudaStream_t stream = nullptr;
     int num_sms = 148;
     bool force_generic = false;      // DGPE_GENERIC=1: runtime-plan kernels only (A/B checks)
+    bool zfast = false;              // warp-per-line z kernels (zline.cuh) and the fused step order z, x, y
 
     cplx* spec = nullptr;                       // [nx][ny][nzh]
     FftPlan plan_x{}, plan_y{}, plan_zh{};      // transform lengths nx, ny, nz/2
@@ -84,6 +86,8 @@ struct dgpe_handle {
     std::vector<cudaEvent_t> prof_ev; // dgpe_step_profile
     std::vector<void*> owned;        // everything to cudaFree
 };
+
+static bool z_specialised(int nz);
 
 static int threads_for(int nbf)
 {
@@ -168,12 +172,12 @@ template <>
 cplx to_ct<cplx>(std::complex<double> z) { return make_double2(z.real(), z.imag()); }
 
 template <typename CT>
-static int build_sweep(dgpe_handle* h, AxisSweep* S, int n, std::complex<double> r)
+static int build_sweep(dgpe_handle* h, AxisSweep* S, int n, std::complex<double> r, int lc)
 {
     typedef std::complex<double> C;
     S->n = n;
     S->r = r;
-    S->Lc = (n <= 514 && !h->force_generic) ? 8 : 16;
+    S->Lc = lc;
     const int nun = n - 2;
     S->G = (nun + S->Lc - 1) / S->Lc;
     std::vector<C> inv(n, C(0)), cc(n, C(0)), F(n, C(0)), Gm(n, C(0)), A(S->G, C(0)), B(S->G, C(0));
@@ -249,6 +253,7 @@ static int init_handle(dgpe_handle* h)
         CU(cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev));
         const char* e = getenv("DGPE_GENERIC");
         h->force_generic = e && e[0] == '1';
+        h->zfast = !h->force_generic && z_specialised(nz);
     }
 
     if ((rc = make_plan(h, nx, &h->plan_x, &h->tw_x))) return rc;
@@ -286,10 +291,14 @@ static int init_handle(dgpe_handle* h)
     const double ds[3] = {h->dx, h->dy, h->dz};
     for (int a = 0; a < 3; ++a) {
         const double rr = h->dt / (4.0 * ds[a] * ds[a]);      // R#9
+        // chunk length of the sweep recursions: 8 (or 16) unknowns per thread on the strided axes; on z
+        // the warp-per-line kernel gives every lane ceil((nz-2)/32) unknowns
+        int lc = (ns[a] <= 514 && !h->force_generic) ? 8 : 16;
+        if (a == 2 && h->zfast) lc = (nz - 2 + 31) / 32;
         if (h->mode == DGPE_IMAG)
-            rc = build_sweep<double>(h, &h->sw[a], ns[a], std::complex<double>(rr, 0.0));
+            rc = build_sweep<double>(h, &h->sw[a], ns[a], std::complex<double>(rr, 0.0), lc);
         else
-            rc = build_sweep<cplx>(h, &h->sw[a], ns[a], std::complex<double>(0.0, rr));
+            rc = build_sweep<cplx>(h, &h->sw[a], ns[a], std::complex<double>(0.0, rr), lc);
         if (rc) return rc;
     }
 
@@ -405,9 +414,116 @@ static int check_launch(const char* what)
     return DGPE_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// warp-per-line z kernels (zline.cuh): specialised line lengths
+// ------------------------------------------------------------------------------------------------
+#define DGPE_Z_SIZES(X) X(64) X(128) X(192) X(256) X(384) X(512) X(768)
+
+static bool z_specialised(int nz)
+{
+    switch (nz) {
+#define X(NN) case NN:
+        DGPE_Z_SIZES(X)
+#undef X
+        return true;
+        default: return false;
+    }
+}
+
+template <int NZ>
+constexpr int z_main_minb(bool use_a, bool use_b)
+{
+    const int per_cta = 4 * ((use_a ? ZGeom<NZ>::A_ELEMS : 0) + (use_b ? ZGeom<NZ>::B_ELEMS : 0)) * 16 + 1024;
+    const int m = (227 * 1024) / per_cta;
+    return m < 1 ? 1 : (m > 4 ? 4 : m);
+}
+
+template <int NZ>
+static int launch_z_r2c_n(dgpe_handle* h, const cplx* psi)
+{
+    constexpr int WARPS = 8;
+    const size_t smem = (size_t)WARPS * ZGeom<NZ>::B_ELEMS * sizeof(cplx);
+    auto kern = k_z_r2c<NZ, WARPS>;
+    static bool ready = false;
+    if (!ready) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ready = true;
+    }
+    const int nlines = h->nx * h->ny;
+    kern<<<(nlines + WARPS - 1) / WARPS, 32 * WARPS, smem, h->stream>>>(psi, h->spec, nlines, h->tw_zh, h->tw_split, h->scal);
+    return check_launch("k_z_r2c");
+}
+
+template <int NZ, typename CT, int SPEC, bool SWEEP>
+static int launch_z_main_n(dgpe_handle* h, cplx* psi, double* phi_out)
+{
+    constexpr int WARPS = 4;
+    constexpr bool USE_A = SPEC != ZS_PHI, USE_B = SPEC != ZS_NONE;
+    constexpr int MINB = z_main_minb<NZ>(USE_A, USE_B);
+    const size_t smem = (size_t)WARPS * ((USE_A ? ZGeom<NZ>::A_ELEMS : 0) + (USE_B ? ZGeom<NZ>::B_ELEMS : 0)) * sizeof(cplx);
+    auto kern = k_z_main<NZ, CT, SPEC, SWEEP, WARPS, MINB>;
+    static bool ready = false;
+    if (!ready) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ready = true;
+    }
+    const AxisSweep& S = h->sw[2];
+    SweepTables<CT> T;
+    T.r = to_ct<CT>(S.r);
+    T.omr2 = to_ct<CT>(1.0 - 2.0 * S.r);
+    T.inv = (const CT*)S.inv; T.cc = (const CT*)S.cc; T.F = (const CT*)S.F; T.Gm = (const CT*)S.Gm;
+    T.Ach = (const CT*)S.Ach; T.Bch = (const CT*)S.Bch;
+    T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb;
+    if (SWEEP && (S.Lc != ZGeom<NZ>::LC || S.G > 32)) return fail(DGPE_ERR_CUDA, "z sweep tables do not match the z-line kernel");
+    ZMainArgs Z;
+    Z.nlines = h->nx * h->ny; Z.ny = h->ny;
+    Z.dt = h->dt; Z.g = h->g; Z.gdd = h->gdd;
+    Z.vx = h->vx; Z.vy = h->vy; Z.vz = h->vz;
+    Z.scal = h->scal; Z.tw = h->tw_zh; Z.tws = h->tw_split; Z.phi_out = phi_out;
+    kern<<<(Z.nlines + WARPS - 1) / WARPS, 32 * WARPS, smem, h->stream>>>(psi, h->spec, Z, T);
+    return check_launch("k_z_main");
+}
+
+// what: 0 = C2R + nonlinear, 1 = C2R + nonlinear + z sweep, 2 = z sweep only, 3 = C2R -> phi_out
+template <int NZ>
+static int launch_z_main_nz(dgpe_handle* h, cplx* psi, int what, double* phi_out)
+{
+    const bool imag = h->mode == DGPE_IMAG;
+    switch (what) {
+        case 0: return imag ? launch_z_main_n<NZ, double, ZS_IMAG, false>(h, psi, nullptr)
+                            : launch_z_main_n<NZ, cplx, ZS_REAL, false>(h, psi, nullptr);
+        case 1: return imag ? launch_z_main_n<NZ, double, ZS_IMAG, true>(h, psi, nullptr)
+                            : launch_z_main_n<NZ, cplx, ZS_REAL, true>(h, psi, nullptr);
+        case 2: return imag ? launch_z_main_n<NZ, double, ZS_NONE, true>(h, psi, nullptr)
+                            : launch_z_main_n<NZ, cplx, ZS_NONE, true>(h, psi, nullptr);
+        default: return launch_z_main_n<NZ, double, ZS_PHI, false>(h, psi, phi_out);
+    }
+}
+
+static int launch_z_main(dgpe_handle* h, cplx* psi, int what, double* phi_out)
+{
+    switch (h->nz) {
+#define X(NN) case NN: return launch_z_main_nz<NN>(h, psi, what, phi_out);
+        DGPE_Z_SIZES(X)
+#undef X
+        default: return fail(DGPE_ERR_UNSUPPORTED, "no z-line kernel for nz = %d", h->nz);
+    }
+}
+
+static int launch_z_r2c(dgpe_handle* h, const cplx* psi)
+{
+    switch (h->nz) {
+#define X(NN) case NN: return launch_z_r2c_n<NN>(h, psi);
+        DGPE_Z_SIZES(X)
+#undef X
+        default: return fail(DGPE_ERR_UNSUPPORTED, "no z-line kernel for nz = %d", h->nz);
+    }
+}
+
 // ---- K1 ----
 static int launch_k1(dgpe_handle* h, const cplx* psi)
 {
+    if (h->zfast) return launch_z_r2c(h, psi);
     const int nlines = h->nx * h->ny, M = h->nz / 2;
     k_dens_r2c<<<(nlines + 7) / 8, threads_for(h->plan_zh.nbf), sizeof(cplx) * TILE_COLS * (size_t)M, h->stream>>>(
         psi, h->spec, nlines, h->nz, h->plan_zh, h->tw_split, h->scal);
@@ -510,6 +626,7 @@ static int launch_dipolar_spectrum(dgpe_handle* h, const cplx* psi)
 // K5 in one of its modes
 static int launch_c2r(dgpe_handle* h, cplx* psi, int kmode, double* out)
 {
+    if (h->zfast && kmode != 2) return launch_z_main(h, psi, kmode == 3 ? 3 : 0, out);
     const int nlines = h->nx * h->ny, M = h->nz / 2;
     NonlinArgs A;
     A.nlines = nlines; A.ny = h->ny; A.nz = h->nz;
@@ -566,6 +683,7 @@ static int launch_sweep_t(dgpe_handle* h, cplx* psi, int axis, bool fold)
 
 static int launch_sweep(dgpe_handle* h, cplx* psi, int axis, bool fold)
 {
+    if (axis == 2 && h->zfast && !fold) return launch_z_main(h, psi, 2, nullptr);
     return h->mode == DGPE_IMAG ? launch_sweep_t<double>(h, psi, axis, fold) : launch_sweep_t<cplx>(h, psi, axis, fold);
 }
 
@@ -575,16 +693,19 @@ static int set_scal(dgpe_handle* h, int clear_bad)
     return check_launch("k_set_scal");
 }
 
-// One step = 8 kernels.  `mark`, if set, is called after each launch with the kernel index.
-static const char* const KERNEL_NAMES[8] = {"K1 dens_r2c(z)", "K2 fft_y fwd", "K3 fft_x*Udd*ifft_x", "K4 fft_y inv",
-                                            "K5 c2r(z)+nonlinear", "K6 sweep_x", "K7 sweep_y", "K8 sweep_z(+norm)"};
+// One step = 8 kernels in the order of the method (K1..K5, sweeps x, y, z), or 7 when the z-line
+// kernels are available: the z sweep then runs fused into K5 and the sweeps go z, x, y (the three 1-D
+// Cayley operators commute: R#26), with the norm folded into the last sweep either way.
+// `mark` is called after each launch with the kernel index.
+static const char* const KERNEL_NAMES8[8] = {"K1 dens_r2c(z)", "K2 fft_y fwd", "K3 fft_x*Udd*ifft_x", "K4 fft_y inv",
+                                             "K5 c2r(z)+nonlinear", "K6 sweep_x", "K7 sweep_y", "K8 sweep_z(+norm)"};
+static const char* const KERNEL_NAMES7[7] = {"K1 dens_r2c(z)", "K2 fft_y fwd", "K3 fft_x*Udd*ifft_x", "K4 fft_y inv",
+                                             "K5+K8 c2r(z)+nonlinear+sweep_z", "K6 sweep_x", "K7 sweep_y(+norm)"};
 
 template <typename Mark>
 static int one_step(dgpe_handle* h, cplx* psi, Mark mark)
 {
     const bool imag = h->mode == DGPE_IMAG;
-    const int nx = h->nx, ny = h->ny, nz = h->nz, nzh = h->nzh, M = nz / 2;
-    const int nlines = nx * ny;
     int rc;
     if ((rc = launch_k1(h, psi))) return rc;
     mark(0);
@@ -594,10 +715,17 @@ static int one_step(dgpe_handle* h, cplx* psi, Mark mark)
     mark(2);
     if ((rc = launch_fft_y(h, true))) return rc;
     mark(3);
-    // K5
+    if (h->zfast) {
+        if ((rc = launch_z_main(h, psi, 1, nullptr))) return rc;
+        mark(4);
+        if ((rc = launch_sweep(h, psi, 0, false))) return rc;
+        mark(5);
+        if ((rc = launch_sweep(h, psi, 1, imag))) return rc;
+        mark(6);
+        return DGPE_OK;
+    }
     if ((rc = launch_c2r(h, psi, imag ? 0 : 1, nullptr))) return rc;
     mark(4);
-    // K6..K8
     if ((rc = launch_sweep(h, psi, 0, false))) return rc;
     mark(5);
     if ((rc = launch_sweep(h, psi, 1, false))) return rc;
@@ -703,10 +831,11 @@ extern "C" int dgpe_step_profile(dgpe_handle* h, void* psi_, int nsteps, double*
 
 extern "C" const char* dgpe_kernel_name(const dgpe_handle* h, int k)
 {
-    (void)h;
-    return (k >= 0 && k < 8) ? KERNEL_NAMES[k] : "";
+    if (!h || k < 0 || k >= dgpe_launches_per_step(h)) return "";
+    return h->zfast ? KERNEL_NAMES7[k] : KERNEL_NAMES8[k];
 }
 
+// algorithmic bytes of kernel k AS BUILT: each array read once and written once per pass
 extern "C" double dgpe_kernel_bytes(const dgpe_handle* h, int k)
 {
     if (!h) return 0.0;
@@ -714,8 +843,9 @@ extern "C" double dgpe_kernel_bytes(const dgpe_handle* h, int k)
     switch (k) {
         case 0: return 16.0 * N + S;       // read psi, write half-spectrum
         case 1: case 2: case 3: return 2.0 * S;
-        case 4: return S + 32.0 * N;       // read spectrum, read + write psi
-        case 5: case 6: case 7: return 32.0 * N;
+        case 4: return S + 32.0 * N;       // read spectrum, read + write psi (the fused z sweep adds no traffic)
+        case 5: case 6: return 32.0 * N;
+        case 7: return h->zfast ? 0.0 : 32.0 * N;
         default: return 0.0;
     }
 }
@@ -845,6 +975,5 @@ extern "C" double dgpe_bytes_per_step(const dgpe_handle* h)
 
 extern "C" int dgpe_launches_per_step(const dgpe_handle* h)
 {
-    (void)h;
-    return 8;
+    return (h && h->zfast) ? 7 : 8;
 }

@@ -1,0 +1,297 @@
+// zline.cuh -- the kernels of the contiguous axis z for the specialised line lengths, one WARP per
+// z-line (SV section 8a rows a1, a5, a8; BJ:north_star "the R2C density transform fused with the
+// |psi|^2 computation on load", "the nonlinear exponential update fused into the inverse-last pass",
+// "for the z sweep, the contiguous axis, tiles are ... staged in shared memory so the recursion runs
+// along a transposed tile").
+//
+// A z-line is contiguous in global memory, so a warp reads and writes it with fully coalesced 512-byte
+// accesses and needs no neighbouring lines: every line is an independent job of one warp, synchronised
+// with __syncwarp only.  Many warps per SM (16 at 512^3) are in different phases at any time, which
+// overlaps the loads, the shared-memory passes, the fp64 arithmetic and the stores without block
+// barriers.
+//
+//   k_z_r2c   (K1)   n = s2 |psi|^2 -> packed nz/2-point FFT -> Hermitian split -> nz/2+1 bins
+//   k_z_main  (K5, K8, or both fused) Hermitian merge -> nz/2-point inverse FFT = Phi -> nonlinear
+//             exponential -> Crank-Nicolson sweep along z with the chunk of each lane in registers
+//
+// Shared memory per warp:
+//   B  FFT buffer, M = nz/2 complex, element idx at idx + (idx >> 3)  (the one pad per 8 elements makes
+//      the stride-R writes of the first pass conflict free);
+//   A  the psi line for the sweep, element j >= 1 at 1 + PITCH*((j-1)/LC) + (j-1)%LC, element 0 at 0:
+//      lane l owns the LC unknowns 1 + l LC .. of the Thomas recursions and PITCH = LC | 1 is odd, so the
+//      per-lane walks along a chunk and the coalesced walks along the line are both conflict free.
+#pragma once
+#include "ctfft.cuh"
+#include "sweep.cuh"
+
+namespace dgpe {
+
+template <int NZ>
+struct ZGeom {
+    static constexpr int M = NZ / 2;
+    static constexpr int NPER = NZ / 32;                 // psi elements per lane
+    static constexpr int LC = (NZ - 2 + 31) / 32;        // sweep chunk per lane
+    static constexpr int PITCH = LC | 1;
+    static constexpr int A_ELEMS = (1 + 32 * PITCH + 7) / 8 * 8;
+    static constexpr int B_ELEMS = (M + (M >> 3) + 7) / 8 * 8;
+    static_assert(NZ % 64 == 0, "z-line kernels need nz to be a multiple of 64");
+};
+
+struct PosPad {
+    static __device__ __forceinline__ int at(int idx) { return idx + (idx >> 3); }
+};
+
+template <int NZ>
+struct PosLine {
+    static __device__ __forceinline__ int at(int j)
+    {
+        constexpr int LC = ZGeom<NZ>::LC, PITCH = ZGeom<NZ>::PITCH;
+        const int q = (j - 1) / LC;
+        return (j == 0) ? 0 : 1 + PITCH * q + (j - 1 - q * LC);
+    }
+};
+
+__device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+__device__ __forceinline__ cplx shfl_c(cplx v, int src) { return mk(shfl_d(v.x, src), shfl_d(v.y, src)); }
+__device__ __forceinline__ double shfl_ct(double v, int src) { return shfl_d(v, src); }
+__device__ __forceinline__ cplx shfl_ct(cplx v, int src) { return shfl_c(v, src); }
+__device__ __forceinline__ double ct_zero(double) { return 0.0; }
+__device__ __forceinline__ cplx ct_zero(cplx) { return mk(0.0, 0.0); }
+
+// ------------------------------------------------------------------------------------------------
+// K1: density + real-to-complex transform along z.  With M = nz/2 the real line is packed as
+// z_m = n_{2m} + i n_{2m+1}; Z = DFT_M(z); X_k = (Z_k + conj Z_{M-k})/2 - (i/2) e^{-2 pi i k/nz}
+// (Z_k - conj Z_{M-k}), k = 0..M, Z_M := Z_0.   tws[k] = exp(-2 pi i k/nz).
+// grid = ceil(nlines / WARPS); block = 32*WARPS; dynamic shared memory = WARPS * B_ELEMS * 16 bytes.
+// ------------------------------------------------------------------------------------------------
+template <int NZ, int WARPS>
+__global__ void __launch_bounds__(32 * WARPS)
+k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const cplx* __restrict__ tw,
+        const cplx* __restrict__ tws, const double* __restrict__ scal)
+{
+    using G = ZGeom<NZ>;
+    constexpr int M = G::M, L = ct::npass(M);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int line = blockIdx.x * WARPS + warp;
+    if (line >= nlines) return;                         // warps are independent: no block barrier below
+    cplx* B = reinterpret_cast<cplx*>(smem_raw) + (size_t)warp * G::B_ELEMS;
+    double* Bd = reinterpret_cast<double*>(B);
+    const double s2 = scal[SC_S2];
+
+    const cplx* p = psi + (long long)line * NZ;
+    cplx a[G::NPER];
+#pragma unroll
+    for (int i = 0; i < G::NPER; ++i) a[i] = ld_stream(p + 32 * i + lane);
+#pragma unroll
+    for (int i = 0; i < G::NPER; ++i) {
+        const int e = 32 * i + lane, m = e >> 1;
+        Bd[2 * PosPad::at(m) + (e & 1)] = s2 * cabs2(a[i]);
+    }
+    __syncwarp();
+
+    auto none = [](int) { return mk(0.0, 0.0); };
+    ct_fft_range<M, false, false, 32, SyncWarp, PosPad, 0, L, false>(
+        B, lane, true, tw, none, [&](int idx, cplx v) { B[PosPad::at(idx)] = v; });
+    __syncwarp();
+
+    cplx* out = spec + (long long)line * (M + 1);
+    auto split = [&](int k) {
+        const int k1 = (k == M) ? 0 : k, k2 = (k == 0) ? 0 : M - k;
+        const cplx zk = B[PosPad::at(k1)];
+        const cplx zm = cconj(B[PosPad::at(k2)]);
+        const cplx w = __ldg(&tws[k]);
+        const cplx s = cadd(zk, zm), d = csub(zk, zm);
+        const cplx wd = cmul(w, d);
+        st_stream(out + k, mk(0.5 * (s.x + wd.y), 0.5 * (s.y - wd.x)));     // s/2 - (i/2) w d
+    };
+#pragma unroll
+    for (int t = 0; t < M / 32; ++t) split(lane + 32 * t);
+    if (lane == 0) split(M);
+}
+
+// ------------------------------------------------------------------------------------------------
+// K5 / K8: everything that happens to one z-line of psi between two strided passes.
+//   SPEC = ZS_NONE    only the sweep (dgpe_sweep along z)
+//   SPEC = ZS_IMAG    C2R + psi <- exp(-dt H) s1 psi              (BJ:north_star (b), imaginary time)
+//   SPEC = ZS_REAL    C2R + psi <- (cos(dt H) - i sin(dt H)) psi  (real time)
+//   SPEC = ZS_PHI     C2R, Phi written to phi_out (dgpe_dipolar); psi untouched
+//   SWEEP             followed by the Crank-Nicolson sweep along z of the same line while it is still
+//                     in shared memory (the three 1-D Cayley operators commute, so the step may run
+//                     its sweeps in the order z, x, y: DESIGN.md R#26) -- this removes one full
+//                     read+write pass over psi (32N bytes) from the step.
+// C2R: from the half-spectrum X_0..X_M of the line, Z_k = (X_k + conj X_{M-k}) + i e^{+2 pi i k/nz}
+// (X_k - conj X_{M-k}), k = 0..M-1; z = IDFT_M(Z) (the 1/N is already in K3); Phi_{2m} = Re z_m,
+// Phi_{2m+1} = Im z_m.   H = V + g n + gdd Phi, n = s2 |psi|^2, V = (vx[i] + vy[j] + vz[k])/2.
+// Sweep: as sweep.cuh; lane l owns the unknowns 1 + l LC .. and keeps them in registers through the
+// forward elimination, the back substitution and the fix-up; the chunk outflows travel by shuffles.
+// grid = ceil(nlines / WARPS); block = 32*WARPS; dynamic smem = WARPS*(A_ELEMS + B_ELEMS)*16 bytes.
+// ------------------------------------------------------------------------------------------------
+enum { ZS_NONE = 0, ZS_IMAG = 1, ZS_REAL = 2, ZS_PHI = 3 };
+
+struct ZMainArgs {
+    int nlines, ny;
+    double dt, g, gdd;
+    const double *vx, *vy, *vz;
+    const double* scal;
+    const cplx* tw;        // exp(-2 pi i j/M)
+    const cplx* tws;       // exp(-2 pi i k/nz)
+    double* phi_out;       // ZS_PHI
+};
+
+template <int NZ, typename CT, int SPEC, bool SWEEP, int WARPS, int MINB>
+__global__ void __launch_bounds__(32 * WARPS, MINB)
+k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, SweepTables<CT> T)
+{
+    using G = ZGeom<NZ>;
+    using PL = PosLine<NZ>;
+    constexpr int M = G::M, L = ct::npass(M), LC = G::LC;
+    constexpr bool USE_A = (SPEC != ZS_PHI);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int line = blockIdx.x * WARPS + warp;
+    if (line >= Z.nlines) return;                       // warps are independent: no block barrier below
+    constexpr int PER_WARP = (USE_A ? G::A_ELEMS : 0) + (SPEC != ZS_NONE ? G::B_ELEMS : 0);
+    cplx* A = reinterpret_cast<cplx*>(smem_raw) + (size_t)warp * PER_WARP;
+    cplx* B = A + (USE_A ? G::A_ELEMS : 0);
+    cplx* p = psi + (long long)line * NZ;
+
+    // ---- stage the psi line (asynchronous: overlaps the spectrum loads and the merge) ----
+    if constexpr (USE_A) {
+#pragma unroll
+        for (int i = 0; i < G::NPER; ++i) {
+            const int e = 32 * i + lane;
+            cp_async16(&A[PL::at(e)], p + e);
+        }
+        cp_async_commit();
+    }
+
+    if constexpr (SPEC != ZS_NONE) {
+        // ---- Hermitian merge straight from global memory into the FFT buffer ----
+        const cplx* in = spec + (long long)line * (M + 1);
+        cplx xa[M / 32], xb[M / 32];
+#pragma unroll
+        for (int t = 0; t < M / 32; ++t) {
+            const int k = lane + 32 * t;
+            xa[t] = __ldcs(reinterpret_cast<const double2*>(in + k));
+            xb[t] = __ldcs(reinterpret_cast<const double2*>(in + (M - k)));
+        }
+#pragma unroll
+        for (int t = 0; t < M / 32; ++t) {
+            const int k = lane + 32 * t;
+            const cplx w = cconj(__ldg(&Z.tws[k]));               // e^{+2 pi i k/nz}
+            const cplx cb = cconj(xb[t]);
+            const cplx s = cadd(xa[t], cb), d = csub(xa[t], cb);
+            const cplx wd = cmul(w, d);
+            B[PosPad::at(k)] = mk(s.x - wd.y, s.y + wd.x);        // s + i w d
+        }
+    }
+    if constexpr (USE_A) cp_async_wait<0>();
+    __syncwarp();
+
+    if constexpr (SPEC != ZS_NONE) {
+        const int i = line / Z.ny, j = line - i * Z.ny;
+        const double vxy = __ldg(&Z.vx[i]) + __ldg(&Z.vy[j]);
+        const double s2 = Z.scal[SC_S2], s1 = Z.scal[SC_S1];
+        auto none = [](int) { return mk(0.0, 0.0); };
+        ct_fft_range<M, true, false, 32, SyncWarp, PosPad, 0, L, false>(B, lane, true, Z.tw, none, [&](int m, cplx phi) {
+            if constexpr (SPEC == ZS_PHI) {
+                reinterpret_cast<double2*>(Z.phi_out + (long long)line * NZ)[m] = phi;
+            } else {
+                const double2 vz = __ldg(reinterpret_cast<const double2*>(Z.vz) + m);
+                const double vzz[2] = {vz.x, vz.y}, ph[2] = {phi.x, phi.y};
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                    const int pos = PL::at(2 * m + t);
+                    cplx a = A[pos];
+                    const double dens = s2 * cabs2(a);
+                    const double H = 0.5 * (vxy + vzz[t]) + Z.g * dens + Z.gdd * ph[t];
+                    if constexpr (SPEC == ZS_IMAG) {
+                        const double f = exp(-Z.dt * H) * s1;
+                        a = mk(f * a.x, f * a.y);
+                    } else {
+                        double sn, cs;
+                        sincos(Z.dt * H, &sn, &cs);
+                        a = mk(cs * a.x + sn * a.y, cs * a.y - sn * a.x);
+                    }
+                    A[pos] = a;
+                }
+            }
+        });
+        __syncwarp();
+    }
+
+    if constexpr (SWEEP) {
+        const int s = 1 + lane * LC;
+        const int cnt = min(LC, NZ - 1 - s);              // unknowns of this lane's chunk (<= 0: idle lane)
+        const int Gn = T.G;
+        // ---- A: local forward elimination with zero inflow; end nodes read as zero (R#7, R#8) ----
+        cplx ev[LC];
+        cplx e = mk(0.0, 0.0);
+        {
+            cplx pm = (lane == 0 || cnt <= 0) ? mk(0.0, 0.0) : A[PL::at(s - 1)];
+            cplx p0 = (cnt > 0) ? A[PL::at(s)] : mk(0.0, 0.0);
+#pragma unroll
+            for (int i = 0; i < LC; ++i) {
+                ev[i] = mk(0.0, 0.0);
+                if (i < cnt) {
+                    const int jn = s + i + 1;
+                    const cplx pp = (jn < NZ - 1) ? A[PL::at(jn)] : mk(0.0, 0.0);
+                    cplx d = coef_mul(T.r, cadd(pm, pp));
+                    d = coef_fma(T.omr2, p0, d);
+                    d = coef_fma(T.r, e, d);
+                    e = coef_mul(__ldg(&T.inv[s + i]), d);
+                    ev[i] = e;
+                    pm = p0;
+                    p0 = pp;
+                }
+            }
+        }
+        // ---- B: forward inflow by a look-back over the lanes to the left ----
+        const CT Ag = (lane < Gn) ? __ldg(&T.Ach[lane]) : ct_zero(CT());
+        const CT Bg = (lane < Gn) ? __ldg(&T.Bch[lane]) : ct_zero(CT());
+        cplx ein = mk(0.0, 0.0);
+        for (int d = T.Kf; d >= 1; --d) {
+            const int h = lane - d;
+            const cplx Eh = shfl_c(e, h & 31);
+            const CT Ah = shfl_ct(Ag, h & 31);
+            if (h >= 0) ein = coef_fma(Ah, ein, Eh);
+        }
+        // ---- C: local back substitution with zero inflow ----
+        cplx x = mk(0.0, 0.0);
+#pragma unroll
+        for (int i = LC - 1; i >= 0; --i) {
+            if (i < cnt) {
+                const cplx ee = coef_fma(__ldg(&T.F[s + i]), ein, ev[i]);
+                x = csub(ee, coef_mul(__ldg(&T.cc[s + i]), x));
+                ev[i] = x;
+            }
+        }
+        // ---- D: backward inflow from the lanes to the right ----
+        cplx xin = mk(0.0, 0.0);
+        for (int d = T.Kb; d >= 1; --d) {
+            const int h = lane + d;
+            const cplx Xh = shfl_c(x, h & 31);
+            const CT Bh = shfl_ct(Bg, h & 31);
+            if (h < Gn) xin = coef_fma(Bh, xin, Xh);
+        }
+        __syncwarp();                                    // every lane has read its neighbours' values
+        // ---- E: final values back into the line buffer; Dirichlet end nodes are exact zeros ----
+#pragma unroll
+        for (int i = 0; i < LC; ++i)
+            if (i < cnt) A[PL::at(s + i)] = coef_fma(__ldg(&T.Gm[s + i]), xin, ev[i]);
+        if (lane == 0) A[PL::at(0)] = mk(0.0, 0.0);
+        if (lane == 31) A[PL::at(NZ - 1)] = mk(0.0, 0.0);
+        __syncwarp();
+    }
+
+    if constexpr (USE_A) {
+#pragma unroll
+        for (int i = 0; i < G::NPER; ++i) {
+            const int e = 32 * i + lane;
+            st_stream(p + e, A[PL::at(e)]);
+        }
+    }
+}
+
+}  // namespace dgpe
