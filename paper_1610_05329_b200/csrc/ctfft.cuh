@@ -78,13 +78,24 @@ struct CtPass {
 #pragma unroll
                 for (int q = 0; q < R; ++q) v[u][q] = f(j + q * NBUT);
                 if (Ns > 1) {
+                    // twiddles w^q, w = tw[k TWSTEP]: the powers 1, 2, 4 come from the fp64 table, the
+                    // others are one product of two table entries (<= 3 ulp), which trades 4 of the 7
+                    // table loads of a radix-8 butterfly for 4 complex multiplications
                     const int k = j % Ns;
+                    cplx w[R];
 #pragma unroll
-                    for (int q = 1; q < R; ++q) {
-                        cplx w = __ldg(&tw[q * k * TWSTEP]);
-                        if (INV) w.y = -w.y;
-                        v[u][q] = cmul(v[u][q], w);
+                    for (int q = 1; q < R; q <<= 1) {
+                        w[q] = __ldg(&tw[q * k * TWSTEP]);
+                        if (INV) w[q].y = -w[q].y;
                     }
+                    if (R >= 4) w[3] = cmul(w[1], w[2]);
+                    if (R == 8) {
+                        w[5] = cmul(w[1], w[4]);
+                        w[6] = cmul(w[2], w[4]);
+                        w[7] = cmul(w[3], w[4]);
+                    }
+#pragma unroll
+                    for (int q = 1; q < R; ++q) v[u][q] = cmul(v[u][q], w[q]);
                 }
             }
         }

@@ -51,7 +51,7 @@ extern "C" const char* dgpe_last_error(void) { return g_err; }
 // handle
 // ------------------------------------------------------------------------------------------------
 struct AxisSweep {
-    int n = 0, Lc = 0, G = 0, Kf = 0, Kb = 0;
+    int n = 0, Lc = 0, G = 0, Kf = 0, Kb = 0, gU = 0;
     std::complex<double> r;
     void* inv = nullptr;   // device tables, double (imag) or cplx (real)
     void* cc = nullptr;
@@ -199,6 +199,17 @@ static int build_sweep(dgpe_handle* h, AxisSweep* S, int n, std::complex<double>
         B[g] = acc;
         amax = std::max(amax, std::abs(A[g]));
         bmax = std::max(bmax, std::abs(B[g]));
+    }
+    // first chunk from which all full interior chunks (.. G-2) carry bit-identical table entries
+    S->gU = S->G;
+    for (int c0 = 0; c0 + 1 < S->G; ++c0) {
+        bool same = true;
+        for (int g = c0 + 1; g <= S->G - 2 && same; ++g)
+            for (int i = 0; i < S->Lc && same; ++i) {
+                const int a = 1 + c0 * S->Lc + i, b = 1 + g * S->Lc + i;
+                same = inv[a] == inv[b] && cc[a] == cc[b] && F[a] == F[b] && Gm[a] == Gm[b];
+            }
+        if (same) { S->gU = c0; break; }
     }
     const double tol = std::ldexp(1.0, -80);
     auto depth = [&](double q) {
@@ -473,7 +484,7 @@ static int launch_z_main_n(dgpe_handle* h, cplx* psi, double* phi_out)
     T.omr2 = to_ct<CT>(1.0 - 2.0 * S.r);
     T.inv = (const CT*)S.inv; T.cc = (const CT*)S.cc; T.F = (const CT*)S.F; T.Gm = (const CT*)S.Gm;
     T.Ach = (const CT*)S.Ach; T.Bch = (const CT*)S.Bch;
-    T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb;
+    T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb; T.gU = S.gU;
     if (SWEEP && (S.Lc != ZGeom<NZ>::LC || S.G > 32)) return fail(DGPE_ERR_CUDA, "z sweep tables do not match the z-line kernel");
     ZMainArgs Z;
     Z.nlines = h->nx * h->ny; Z.ny = h->ny;
@@ -654,7 +665,7 @@ static int launch_sweep_t(dgpe_handle* h, cplx* psi, int axis, bool fold)
     T.omr2 = to_ct<CT>(1.0 - 2.0 * S.r);
     T.inv = (const CT*)S.inv; T.cc = (const CT*)S.cc; T.F = (const CT*)S.F; T.Gm = (const CT*)S.Gm;
     T.Ach = (const CT*)S.Ach; T.Bch = (const CT*)S.Bch;
-    T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb;
+    T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb; T.gU = S.gU;
     SweepFold F;
     F.enabled = fold ? 1 : 0;
     F.dV = h->dx * h->dy * h->dz;

@@ -43,6 +43,8 @@ struct SweepTables {
     const CT* Ach;     // [G]   chunk forward factor
     const CT* Bch;     // [G]   chunk backward factor
     int Lc, G, Kf, Kb;
+    int gU;            // chunks gU .. G-2 have bit-identical table entries (G if none): a lane-per-chunk kernel
+                       // may read chunk gU's entries for all of them (one broadcast address)
 };
 
 struct SweepFold {

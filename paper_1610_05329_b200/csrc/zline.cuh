@@ -225,6 +225,10 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         const int s = 1 + lane * LC;
         const int cnt = min(LC, NZ - 1 - s);              // unknowns of this lane's chunk (<= 0: idle lane)
         const int Gn = T.G;
+        // table base of this lane: away from the left wall the elimination factors have converged to
+        // their fixed point, so the interior chunks share one set of entries (T.gU, decided on the host
+        // by a bitwise comparison) -- one broadcast address per load instead of 32 scattered ones
+        const int sT = (lane >= T.gU && lane < Gn - 1) ? 1 + T.gU * LC : s;
         // ---- A: local forward elimination with zero inflow; end nodes read as zero (R#7, R#8) ----
         cplx ev[LC];
         cplx e = mk(0.0, 0.0);
@@ -240,7 +244,7 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
                     cplx d = coef_mul(T.r, cadd(pm, pp));
                     d = coef_fma(T.omr2, p0, d);
                     d = coef_fma(T.r, e, d);
-                    e = coef_mul(__ldg(&T.inv[s + i]), d);
+                    e = coef_mul(__ldg(&T.inv[sT + i]), d);
                     ev[i] = e;
                     pm = p0;
                     p0 = pp;
@@ -262,8 +266,8 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
 #pragma unroll
         for (int i = LC - 1; i >= 0; --i) {
             if (i < cnt) {
-                const cplx ee = coef_fma(__ldg(&T.F[s + i]), ein, ev[i]);
-                x = csub(ee, coef_mul(__ldg(&T.cc[s + i]), x));
+                const cplx ee = coef_fma(__ldg(&T.F[sT + i]), ein, ev[i]);
+                x = csub(ee, coef_mul(__ldg(&T.cc[sT + i]), x));
                 ev[i] = x;
             }
         }
@@ -279,7 +283,7 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         // ---- E: final values back into the line buffer; Dirichlet end nodes are exact zeros ----
 #pragma unroll
         for (int i = 0; i < LC; ++i)
-            if (i < cnt) A[PL::at(s + i)] = coef_fma(__ldg(&T.Gm[s + i]), xin, ev[i]);
+            if (i < cnt) A[PL::at(s + i)] = coef_fma(__ldg(&T.Gm[sT + i]), xin, ev[i]);
         if (lane == 0) A[PL::at(0)] = mk(0.0, 0.0);
         if (lane == 31) A[PL::at(NZ - 1)] = mk(0.0, 0.0);
         __syncwarp();
