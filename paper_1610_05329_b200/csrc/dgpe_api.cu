@@ -59,6 +59,8 @@ struct AxisSweep {
     void* Gm = nullptr;
     void* Ach = nullptr;
     void* Bch = nullptr;
+    std::vector<std::complex<double>> h_inv, h_cc, h_F, h_Gm;   // host copies (kernel-parameter tables of the z sweep)
+    bool consttab = false;   // chunk 0 + one converged chunk describe the whole line (zline.cuh ZTabs)
 };
 
 struct dgpe_handle {
@@ -211,6 +213,17 @@ static int build_sweep(dgpe_handle* h, AxisSweep* S, int n, std::complex<double>
             }
         if (same) { S->gU = c0; break; }
     }
+    S->consttab = (S->G == 1);
+    if (S->G >= 2 && S->gU <= 1) {
+        bool same = true;
+        const int g = S->G - 1;
+        for (int i = 0; i < S->Lc && 1 + g * S->Lc + i <= n - 2 && same; ++i) {
+            const int a = 1 + S->Lc + i, b = 1 + g * S->Lc + i;
+            same = inv[a] == inv[b] && cc[a] == cc[b] && F[a] == F[b];
+        }
+        S->consttab = same;
+    }
+    S->h_inv = inv; S->h_cc = cc; S->h_F = F; S->h_Gm = Gm;
     const double tol = std::ldexp(1.0, -80);
     auto depth = [&](double q) {
         int K = 1;
@@ -465,14 +478,14 @@ static int launch_z_r2c_n(dgpe_handle* h, const cplx* psi)
     return check_launch("k_z_r2c");
 }
 
-template <int NZ, typename CT, int SPEC, bool SWEEP>
-static int launch_z_main_n(dgpe_handle* h, cplx* psi, double* phi_out)
+template <int NZ, typename CT, int SPEC, bool SWEEP, bool CONSTTAB>
+static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
 {
-    constexpr int WARPS = 4;
+    constexpr int WARPS = 4, LC = ZGeom<NZ>::LC;
     constexpr bool USE_A = SPEC != ZS_PHI, USE_B = SPEC != ZS_NONE;
     constexpr int MINB = z_main_minb<NZ>(USE_A, USE_B);
     const size_t smem = (size_t)WARPS * ((USE_A ? ZGeom<NZ>::A_ELEMS : 0) + (USE_B ? ZGeom<NZ>::B_ELEMS : 0)) * sizeof(cplx);
-    auto kern = k_z_main<NZ, CT, SPEC, SWEEP, WARPS, MINB>;
+    auto kern = k_z_main<NZ, CT, SPEC, SWEEP, CONSTTAB, WARPS, MINB>;
     static bool ready = false;
     if (!ready) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -485,14 +498,34 @@ static int launch_z_main_n(dgpe_handle* h, cplx* psi, double* phi_out)
     T.inv = (const CT*)S.inv; T.cc = (const CT*)S.cc; T.F = (const CT*)S.F; T.Gm = (const CT*)S.Gm;
     T.Ach = (const CT*)S.Ach; T.Bch = (const CT*)S.Bch;
     T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb; T.gU = S.gU;
-    if (SWEEP && (S.Lc != ZGeom<NZ>::LC || S.G > 32)) return fail(DGPE_ERR_CUDA, "z sweep tables do not match the z-line kernel");
+    if (SWEEP && (S.Lc != LC || S.G > 32)) return fail(DGPE_ERR_CUDA, "z sweep tables do not match the z-line kernel");
+    ZTabs<CT, LC> P;
+    std::memset(&P, 0, sizeof(P));
+    if (SWEEP && CONSTTAB) {
+        const int n = h->nz, u0 = (S.G >= 2) ? 1 + LC : 1;
+        for (int i = 0; i < LC; ++i) {
+            const int a = std::min(1 + i, n - 1), b = std::min(u0 + i, n - 1);     // entries past n-2 are zero and unused
+            P.inv0[i] = to_ct<CT>(S.h_inv[a]); P.cc0[i] = to_ct<CT>(S.h_cc[a]); P.gm0[i] = to_ct<CT>(S.h_Gm[a]);
+            P.invU[i] = to_ct<CT>(S.h_inv[b]); P.ccU[i] = to_ct<CT>(S.h_cc[b]);
+            P.fU[i] = to_ct<CT>(S.h_F[b]); P.gmU[i] = to_ct<CT>(S.h_Gm[b]);
+        }
+    }
     ZMainArgs Z;
     Z.nlines = h->nx * h->ny; Z.ny = h->ny;
     Z.dt = h->dt; Z.g = h->g; Z.gdd = h->gdd;
     Z.vx = h->vx; Z.vy = h->vy; Z.vz = h->vz;
     Z.scal = h->scal; Z.tw = h->tw_zh; Z.tws = h->tw_split; Z.phi_out = phi_out;
-    kern<<<(Z.nlines + WARPS - 1) / WARPS, 32 * WARPS, smem, h->stream>>>(psi, h->spec, Z, T);
+    kern<<<(Z.nlines + WARPS - 1) / WARPS, 32 * WARPS, smem, h->stream>>>(psi, h->spec, Z, T, P);
     return check_launch("k_z_main");
+}
+
+template <int NZ, typename CT, int SPEC, bool SWEEP>
+static int launch_z_main_n(dgpe_handle* h, cplx* psi, double* phi_out)
+{
+    if constexpr (SWEEP) {
+        if (h->sw[2].consttab) return launch_z_main_c<NZ, CT, SPEC, true, true>(h, psi, phi_out);
+    }
+    return launch_z_main_c<NZ, CT, SPEC, SWEEP, false>(h, psi, phi_out);
 }
 
 // what: 0 = C2R + nonlinear, 1 = C2R + nonlinear + z sweep, 2 = z sweep only, 3 = C2R -> phi_out

@@ -17,9 +17,9 @@
 // Shared memory per warp:
 //   B  FFT buffer, M = nz/2 complex, element idx at idx + (idx >> 3)  (the one pad per 8 elements makes
 //      the stride-R writes of the first pass conflict free);
-//   A  the psi line for the sweep, element j >= 1 at 1 + PITCH*((j-1)/LC) + (j-1)%LC, element 0 at 0:
-//      lane l owns the LC unknowns 1 + l LC .. of the Thomas recursions and PITCH = LC | 1 is odd, so the
-//      per-lane walks along a chunk and the coalesced walks along the line are both conflict free.
+//   A  the psi line, even and odd elements in two padded halves (PosLine): the coalesced walks along the
+//      line, the pair walk of the nonlinear update and the per-lane walks along a sweep chunk are all
+//      conflict free.
 #pragma once
 #include "ctfft.cuh"
 #include "sweep.cuh"
@@ -31,23 +31,29 @@ struct ZGeom {
     static constexpr int M = NZ / 2;
     static constexpr int NPER = NZ / 32;                 // psi elements per lane
     static constexpr int LC = (NZ - 2 + 31) / 32;        // sweep chunk per lane
-    static constexpr int PITCH = LC | 1;
-    static constexpr int A_ELEMS = (1 + 32 * PITCH + 7) / 8 * 8;
+    static constexpr int HALF = ((M + (M >> 3) + 7) / 8) * 8 + 4;      // offset of the odd half, = 4 mod 8
+    static constexpr int A_ELEMS = (HALF + M + (M >> 3) + 7) / 8 * 8;
     static constexpr int B_ELEMS = (M + (M >> 3) + 7) / 8 * 8;
     static_assert(NZ % 64 == 0, "z-line kernels need nz to be a multiple of 64");
+    static_assert(LC % 2 == 0, "the chunk walk is conflict free only for an even chunk length");
 };
 
 struct PosPad {
     static __device__ __forceinline__ int at(int idx) { return idx + (idx >> 3); }
 };
 
+// Line buffer A: element e = 2m + t lives at t*HALF + m + (m >> 3).  Three access patterns are all
+// free of bank conflicts (16-byte elements: the 8 lanes of a quarter-warp must hit 8 different
+// positions mod 8):  the coalesced walk (lane <-> e), 4 even and 4 odd elements per quarter-warp, the
+// halves 4 banks apart;  the pair walk of the nonlinear update (lane <-> m);  the chunk walk of the
+// sweep (lane <-> e = 1 + LC lane + i, LC even: m advances by LC/2 per lane, the pad makes the stride odd
+// for LC = 16).
 template <int NZ>
 struct PosLine {
-    static __device__ __forceinline__ int at(int j)
+    static __device__ __forceinline__ int at(int e)
     {
-        constexpr int LC = ZGeom<NZ>::LC, PITCH = ZGeom<NZ>::PITCH;
-        const int q = (j - 1) / LC;
-        return (j == 0) ? 0 : 1 + PITCH * q + (j - 1 - q * LC);
+        const int m = e >> 1;
+        return (e & 1) * ZGeom<NZ>::HALF + m + (m >> 3);
     }
 };
 
@@ -139,9 +145,21 @@ struct ZMainArgs {
     double* phi_out;       // ZS_PHI
 };
 
-template <int NZ, typename CT, int SPEC, bool SWEEP, int WARPS, int MINB>
+// Thomas tables of the z sweep as kernel parameters (constant bank: no load instruction at all), valid
+// when the elimination factors have converged by the second chunk (decided on the host, bitwise):
+// lane 0 uses chunk 0's entries, every other lane the converged chunk's.  (The forward inflow of lane 0
+// and the backward inflow of the last lane are zero, so F of chunk 0 and Gm of the last chunk never
+// matter.)  CONSTTAB = false reads the global tables instead (any r).
+template <typename CT, int LC>
+struct ZTabs {
+    CT inv0[LC], cc0[LC], gm0[LC];
+    CT invU[LC], ccU[LC], fU[LC], gmU[LC];
+};
+
+template <int NZ, typename CT, int SPEC, bool SWEEP, bool CONSTTAB, int WARPS, int MINB>
 __global__ void __launch_bounds__(32 * WARPS, MINB)
-k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, SweepTables<CT> T)
+k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, SweepTables<CT> T,
+         const __grid_constant__ ZTabs<CT, ZGeom<NZ>::LC> P)
 {
     using G = ZGeom<NZ>;
     using PL = PosLine<NZ>;
@@ -156,25 +174,29 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
     cplx* B = A + (USE_A ? G::A_ELEMS : 0);
     cplx* p = psi + (long long)line * NZ;
 
-    // ---- stage the psi line (asynchronous: overlaps the spectrum loads and the merge) ----
+    // ---- stage the psi line and merge the half-spectrum; the global loads of both are issued before
+    //      anything waits on them (psi in two batches to bound the registers in flight) ----
+    constexpr int HB = G::NPER / 2;
+    cplx a[HB];
     if constexpr (USE_A) {
 #pragma unroll
-        for (int i = 0; i < G::NPER; ++i) {
-            const int e = 32 * i + lane;
-            cp_async16(&A[PL::at(e)], p + e);
-        }
-        cp_async_commit();
+        for (int i = 0; i < HB; ++i) a[i] = ld_stream(p + 32 * i + lane);
     }
-
     if constexpr (SPEC != ZS_NONE) {
-        // ---- Hermitian merge straight from global memory into the FFT buffer ----
+        // Hermitian merge straight from global memory into the FFT buffer
         const cplx* in = spec + (long long)line * (M + 1);
         cplx xa[M / 32], xb[M / 32];
 #pragma unroll
         for (int t = 0; t < M / 32; ++t) {
             const int k = lane + 32 * t;
-            xa[t] = __ldcs(reinterpret_cast<const double2*>(in + k));
-            xb[t] = __ldcs(reinterpret_cast<const double2*>(in + (M - k)));
+            xa[t] = ld_stream(in + k);
+            xb[t] = ld_stream(in + (M - k));
+        }
+        if constexpr (USE_A) {
+#pragma unroll
+            for (int i = 0; i < HB; ++i) A[PL::at(32 * i + lane)] = a[i];
+#pragma unroll
+            for (int i = 0; i < HB; ++i) a[i] = ld_stream(p + 32 * (HB + i) + lane);
         }
 #pragma unroll
         for (int t = 0; t < M / 32; ++t) {
@@ -185,8 +207,18 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
             const cplx wd = cmul(w, d);
             B[PosPad::at(k)] = mk(s.x - wd.y, s.y + wd.x);        // s + i w d
         }
+        if constexpr (USE_A) {
+#pragma unroll
+            for (int i = 0; i < HB; ++i) A[PL::at(32 * (HB + i) + lane)] = a[i];
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < HB; ++i) A[PL::at(32 * i + lane)] = a[i];
+#pragma unroll
+        for (int i = 0; i < HB; ++i) a[i] = ld_stream(p + 32 * (HB + i) + lane);
+#pragma unroll
+        for (int i = 0; i < HB; ++i) A[PL::at(32 * (HB + i) + lane)] = a[i];
     }
-    if constexpr (USE_A) cp_async_wait<0>();
     __syncwarp();
 
     if constexpr (SPEC != ZS_NONE) {
@@ -229,6 +261,11 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         // their fixed point, so the interior chunks share one set of entries (T.gU, decided on the host
         // by a bitwise comparison) -- one broadcast address per load instead of 32 scattered ones
         const int sT = (lane >= T.gU && lane < Gn - 1) ? 1 + T.gU * LC : s;
+        const bool l0 = lane == 0;
+        auto t_inv = [&](int i) { if constexpr (CONSTTAB) return l0 ? P.inv0[i] : P.invU[i]; else return __ldg(&T.inv[sT + i]); };
+        auto t_cc = [&](int i) { if constexpr (CONSTTAB) return l0 ? P.cc0[i] : P.ccU[i]; else return __ldg(&T.cc[sT + i]); };
+        auto t_F = [&](int i) { if constexpr (CONSTTAB) return P.fU[i]; else return __ldg(&T.F[sT + i]); };
+        auto t_Gm = [&](int i) { if constexpr (CONSTTAB) return l0 ? P.gm0[i] : P.gmU[i]; else return __ldg(&T.Gm[sT + i]); };
         // ---- A: local forward elimination with zero inflow; end nodes read as zero (R#7, R#8) ----
         cplx ev[LC];
         cplx e = mk(0.0, 0.0);
@@ -244,7 +281,7 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
                     cplx d = coef_mul(T.r, cadd(pm, pp));
                     d = coef_fma(T.omr2, p0, d);
                     d = coef_fma(T.r, e, d);
-                    e = coef_mul(__ldg(&T.inv[sT + i]), d);
+                    e = coef_mul(t_inv(i), d);
                     ev[i] = e;
                     pm = p0;
                     p0 = pp;
@@ -266,8 +303,8 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
 #pragma unroll
         for (int i = LC - 1; i >= 0; --i) {
             if (i < cnt) {
-                const cplx ee = coef_fma(__ldg(&T.F[sT + i]), ein, ev[i]);
-                x = csub(ee, coef_mul(__ldg(&T.cc[sT + i]), x));
+                const cplx ee = coef_fma(t_F(i), ein, ev[i]);
+                x = csub(ee, coef_mul(t_cc(i), x));
                 ev[i] = x;
             }
         }
@@ -283,7 +320,7 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         // ---- E: final values back into the line buffer; Dirichlet end nodes are exact zeros ----
 #pragma unroll
         for (int i = 0; i < LC; ++i)
-            if (i < cnt) A[PL::at(s + i)] = coef_fma(__ldg(&T.Gm[sT + i]), xin, ev[i]);
+            if (i < cnt) A[PL::at(s + i)] = coef_fma(t_Gm(i), xin, ev[i]);
         if (lane == 0) A[PL::at(0)] = mk(0.0, 0.0);
         if (lane == 31) A[PL::at(NZ - 1)] = mk(0.0, 0.0);
         __syncwarp();
