@@ -188,6 +188,10 @@ __device__ __forceinline__ void st_stream(cplx* p, cplx v)
     asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};\n" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
 }
 
+// L2 prefetch of the 128-byte line holding p: kernels ask for the data of the tile / line that will be
+// processed one "residency" later, so that the demand loads of that later CTA hit L2 instead of HBM
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); }
+
 // ---- cp.async (LDGSTS): 16 bytes per thread straight into shared memory, L2-only caching ----
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)

@@ -63,6 +63,8 @@ struct AxisSweep {
     bool consttab = false;   // chunk 0 + one converged chunk describe the whole line (zline.cuh ZTabs)
 };
 
+enum { PF_Z = 1, PF_SWEEP_Y = 2, PF_SWEEP_X = 4, PF_FFT_Y = 8, PF_FFT_X = 16 };
+
 struct dgpe_handle {
     int nx, ny, nz, nzh, mode;
     double dx, dy, dz, dt, gamma, nu, lambda, g, gdd;
@@ -70,6 +72,10 @@ struct dgpe_handle {
     cudaStream_t stream = nullptr;
     int num_sms = 148;
     bool force_generic = false;      // DGPE_GENERIC=1: runtime-plan kernels only (A/B checks)
+    int pf_mult = 1;                 // DGPE_PF_MULT: prefetch distance in units of one residency
+    // L2 prefetch of the next residency, per kernel family (DGPE_PREFETCH=<mask> overrides, for A/B runs):
+    // it pays for the z-line kernels and the y axis; on the x axis (row stride ny*nz) it costs time
+    int prefetch = PF_Z | PF_SWEEP_Y | PF_FFT_Y;
     bool zfast = false;              // warp-per-line z kernels (zline.cuh) and the fused step order z, x, y
 
     cplx* spec = nullptr;                       // [nx][ny][nzh]
@@ -278,6 +284,10 @@ static int init_handle(dgpe_handle* h)
         const char* e = getenv("DGPE_GENERIC");
         h->force_generic = e && e[0] == '1';
         h->zfast = !h->force_generic && z_specialised(nz);
+        const char* pf = getenv("DGPE_PREFETCH");
+        if (pf && pf[0]) h->prefetch = atoi(pf);
+        const char* pm = getenv("DGPE_PF_MULT");
+        if (pm && atoi(pm) > 0) h->pf_mult = atoi(pm);
     }
 
     if ((rc = make_plan(h, nx, &h->plan_x, &h->tw_x))) return rc;
@@ -454,6 +464,21 @@ static bool z_specialised(int nz)
     }
 }
 
+// kernel-parameter copy of the sweep tables: chunk 0 and the converged chunk (sweep.cuh ChunkTabs)
+template <typename CT, int LC>
+static void fill_chunk_tabs(const AxisSweep& S, bool use, ChunkTabs<CT, LC>* P)
+{
+    std::memset(P, 0, sizeof(*P));
+    if (!use) return;
+    const int n = S.n, u0 = (S.G >= 2) ? 1 + LC : 1;
+    for (int i = 0; i < LC; ++i) {
+        const int a = std::min(1 + i, n - 1), b = std::min(u0 + i, n - 1);     // entries past n-2 are zero and unused
+        P->inv0[i] = to_ct<CT>(S.h_inv[a]); P->cc0[i] = to_ct<CT>(S.h_cc[a]); P->gm0[i] = to_ct<CT>(S.h_Gm[a]);
+        P->invU[i] = to_ct<CT>(S.h_inv[b]); P->ccU[i] = to_ct<CT>(S.h_cc[b]);
+        P->fU[i] = to_ct<CT>(S.h_F[b]); P->gmU[i] = to_ct<CT>(S.h_Gm[b]);
+    }
+}
+
 template <int NZ>
 constexpr int z_main_minb(bool use_a, bool use_b)
 {
@@ -499,22 +524,18 @@ static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
     T.Ach = (const CT*)S.Ach; T.Bch = (const CT*)S.Bch;
     T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb; T.gU = S.gU;
     if (SWEEP && (S.Lc != LC || S.G > 32)) return fail(DGPE_ERR_CUDA, "z sweep tables do not match the z-line kernel");
-    ZTabs<CT, LC> P;
-    std::memset(&P, 0, sizeof(P));
-    if (SWEEP && CONSTTAB) {
-        const int n = h->nz, u0 = (S.G >= 2) ? 1 + LC : 1;
-        for (int i = 0; i < LC; ++i) {
-            const int a = std::min(1 + i, n - 1), b = std::min(u0 + i, n - 1);     // entries past n-2 are zero and unused
-            P.inv0[i] = to_ct<CT>(S.h_inv[a]); P.cc0[i] = to_ct<CT>(S.h_cc[a]); P.gm0[i] = to_ct<CT>(S.h_Gm[a]);
-            P.invU[i] = to_ct<CT>(S.h_inv[b]); P.ccU[i] = to_ct<CT>(S.h_cc[b]);
-            P.fU[i] = to_ct<CT>(S.h_F[b]); P.gmU[i] = to_ct<CT>(S.h_Gm[b]);
-        }
-    }
+    ChunkTabs<CT, LC> P;
+    fill_chunk_tabs<CT, LC>(S, SWEEP && CONSTTAB, &P);
     ZMainArgs Z;
     Z.nlines = h->nx * h->ny; Z.ny = h->ny;
     Z.dt = h->dt; Z.g = h->g; Z.gdd = h->gdd;
     Z.vx = h->vx; Z.vy = h->vy; Z.vz = h->vz;
     Z.scal = h->scal; Z.tw = h->tw_zh; Z.tws = h->tw_split; Z.phi_out = phi_out;
+    {
+        static int ctas_per_sm = 0;
+        if (!ctas_per_sm) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, 32 * WARPS, smem));
+        Z.pf_lines = (h->prefetch & PF_Z) ? h->pf_mult * ctas_per_sm * h->num_sms * WARPS : 0;
+    }
     kern<<<(Z.nlines + WARPS - 1) / WARPS, 32 * WARPS, smem, h->stream>>>(psi, h->spec, Z, T, P);
     return check_launch("k_z_main");
 }
@@ -586,7 +607,10 @@ static int launch_fft_xy_n(dgpe_handle* h, const LineMap& map, int nbatch, const
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ready = true;
     }
-    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 1.0 / (double)h->N};
+    static int ctas_per_sm = 0;
+    if (!ctas_per_sm) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, xy_threads<N>(), smem));
+    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 1.0 / (double)h->N,
+              (h->prefetch & (KIND == FFT_X_UDD ? PF_FFT_X : PF_FFT_Y)) ? h->pf_mult * ctas_per_sm * h->num_sms : 0};
     dim3 grid((map.ncols + TILE_COLS - 1) / TILE_COLS, nbatch);
     kern<<<grid, xy_threads<N>(), smem, h->stream>>>(h->spec, map, tw, U);
     return check_launch("k_fft_xy");
@@ -688,6 +712,20 @@ static int launch_c2r(dgpe_handle* h, cplx* psi, int kmode, double* out)
     return check_launch("k_c2r_nonlin");
 }
 
+template <typename CT, int LC, bool CONSTTAB, int MINB>
+static int launch_sweep_xy(dgpe_handle* h, cplx* psi, const LineMap& m, dim3 grid, int thr, const SweepTables<CT>& T,
+                           const SweepFold& F, const AxisSweep& S)
+{
+    auto kern = k_sweep_xy<CT, LC, CONSTTAB, 512, MINB>;
+    ChunkTabs<CT, LC> P;
+    fill_chunk_tabs<CT, LC>(S, CONSTTAB, &P);
+    int ctas_per_sm = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, thr, 0));
+    const int pf = (h->prefetch & (m.batch_stride ? PF_SWEEP_Y : PF_SWEEP_X)) ? h->pf_mult * ctas_per_sm * h->num_sms : 0;
+    kern<<<grid, thr, 0, h->stream>>>(psi, m, T, F, pf, P);
+    return check_launch("k_sweep_xy");
+}
+
 template <typename CT>
 static int launch_sweep_t(dgpe_handle* h, cplx* psi, int axis, bool fold)
 {
@@ -707,9 +745,10 @@ static int launch_sweep_t(dgpe_handle* h, cplx* psi, int axis, bool fold)
     if (axis < 2 && !h->force_generic && S.G <= 64 && (S.Lc == 8 || S.Lc == 16)) {
         LineMap m = axis == 0 ? LineMap{nx, ny * nz, 0, 1, (long long)ny * nz} : LineMap{ny, nz, (long long)ny * nz, 1, nz};
         dim3 grid((m.ncols + TILE_COLS - 1) / TILE_COLS, axis == 0 ? 1 : nx);
-        if (S.Lc == 8) k_sweep_xy<CT, 8, 512, 2><<<grid, thr, 0, h->stream>>>(psi, m, T, F);
-        else k_sweep_xy<CT, 16, 512, 1><<<grid, thr, 0, h->stream>>>(psi, m, T, F);
-        return check_launch("k_sweep_xy");
+        if (S.Lc == 8) return S.consttab ? launch_sweep_xy<CT, 8, true, 2>(h, psi, m, grid, thr, T, F, S)
+                                         : launch_sweep_xy<CT, 8, false, 2>(h, psi, m, grid, thr, T, F, S);
+        return S.consttab ? launch_sweep_xy<CT, 16, true, 1>(h, psi, m, grid, thr, T, F, S)
+                          : launch_sweep_xy<CT, 16, false, 1>(h, psi, m, grid, thr, T, F, S);
     }
     if (axis == 0) {
         LineMap m{nx, ny * nz, 0, 1, (long long)ny * nz};

@@ -47,6 +47,18 @@ struct SweepTables {
                        // may read chunk gU's entries for all of them (one broadcast address)
 };
 
+// The Thomas tables as kernel parameters (constant bank: operands of the fp64 instructions, no load
+// instruction at all), valid when the elimination factors have converged to their fixed point by the
+// second chunk -- decided on the host by a bitwise comparison of the table entries (AxisSweep::consttab).
+// Chunk 0 uses its own entries, every other chunk the converged ones.  The forward inflow of chunk 0
+// and the backward inflow of the last chunk are zero, so F of chunk 0 and Gm of the (possibly shorter)
+// last chunk never matter.  Kernels take CONSTTAB = false to read the global tables instead (any r).
+template <typename CT, int LC>
+struct ChunkTabs {
+    CT inv0[LC], cc0[LC], gm0[LC];
+    CT invU[LC], ccU[LC], fU[LC], gmU[LC];
+};
+
 struct SweepFold {
     int enabled;              // accumulate sum |psi'|^2 and finish the norm in the last block
     double dV;

@@ -23,6 +23,7 @@ struct UddArgs {
     int nzh;                          // kz bins per row of the half-spectrum
     const double *kx2, *ky2, *kz2;    // squared wave numbers (R#10, R#11)
     double invN;                      // 1/(nx ny nz): normalisation of the inverse transform (R#10)
+    int pf_tiles;                     // L2 prefetch distance in tiles (one residency of CTAs); 0 = off
 };
 
 enum { FFT_FWD = 0, FFT_INV = 1, FFT_X_UDD = 2 };
@@ -60,6 +61,18 @@ k_fft_xy(cplx* __restrict__ data, LineMap map, const cplx* __restrict__ tw, UddA
     cplx* g = data + (long long)blockIdx.y * map.batch_stride + (long long)(colok ? col : 0) * map.col_stride;
     const long long es = map.elem_stride;
     cplx* colsm = reinterpret_cast<cplx*>(smem_raw) + c;
+    if (U.pf_tiles > 0) {
+        // ask L2 for the tile a CTA will process one residency later (rows of 128 bytes, which straddle
+        // two lines when the half-spectrum row length nz/2+1 is odd)
+        const long long id = (long long)blockIdx.y * gridDim.x + blockIdx.x + U.pf_tiles;
+        const int by = (int)(id / gridDim.x), bx = (int)(id - (long long)by * gridDim.x);
+        if (by < (int)gridDim.y) {
+            const char* t0 = reinterpret_cast<const char*>(data + (long long)by * map.batch_stride +
+                                                           (long long)bx * TILE_COLS * map.col_stride);
+            for (int j = tid; j < 2 * N; j += xy_threads<N>())
+                prefetch_l2(t0 + (long long)(j >> 1) * es * 16 + (j & 1) * 112);
+        }
+    }
     auto from_g = [&](int idx) { return ld_stream(g + (long long)idx * es); };
     auto to_g = [&](int idx, cplx v) { st_stream(g + (long long)idx * es, v); };
 

@@ -22,9 +22,11 @@
 namespace dgpe {
 
 // grid = (ceil(ncols/8), nbatch); block = 8*G rounded up to a warp multiple (<= NTMAX)
-template <typename CT, int LC, int NTMAX, int MINB>
+// pf_tiles > 0: every CTA asks L2 for the tile that will be processed pf_tiles CTAs later.
+template <typename CT, int LC, bool CONSTTAB, int NTMAX, int MINB>
 __global__ void __launch_bounds__(NTMAX, MINB)
-k_sweep_xy(cplx* __restrict__ psi, LineMap map, SweepTables<CT> T, SweepFold fold)
+k_sweep_xy(cplx* __restrict__ psi, LineMap map, SweepTables<CT> T, SweepFold fold, int pf_tiles,
+           const __grid_constant__ ChunkTabs<CT, LC> P)
 {
     __shared__ cplx smE[NTMAX / 8][TILE_COLS];
     __shared__ cplx smX[NTMAX / 8][TILE_COLS];
@@ -39,6 +41,19 @@ k_sweep_xy(cplx* __restrict__ psi, LineMap map, SweepTables<CT> T, SweepFold fol
     const int cnt = t_end - s;                     // unknowns of this chunk (<= 0 for idle threads)
     cplx* gp = psi + (long long)blockIdx.y * map.batch_stride + (long long)(colok ? col : 0) * map.col_stride;
     const long long es = map.elem_stride;
+
+    if (pf_tiles > 0) {
+        const long long id = (long long)blockIdx.y * gridDim.x + blockIdx.x + pf_tiles;
+        const int by = (int)(id / gridDim.x), bx = (int)(id - (long long)by * gridDim.x);
+        if (by < (int)gridDim.y)
+            for (int j = tid; j < n; j += blockDim.x)
+                prefetch_l2(psi + (long long)by * map.batch_stride + (long long)bx * TILE_COLS * map.col_stride + (long long)j * es);
+    }
+    const bool g0 = g == 0;
+    auto t_inv = [&](int i) { if constexpr (CONSTTAB) return g0 ? P.inv0[i] : P.invU[i]; else return __ldg(&T.inv[s + i]); };
+    auto t_cc = [&](int i) { if constexpr (CONSTTAB) return g0 ? P.cc0[i] : P.ccU[i]; else return __ldg(&T.cc[s + i]); };
+    auto t_F = [&](int i) { if constexpr (CONSTTAB) return P.fU[i]; else return __ldg(&T.F[s + i]); };
+    auto t_Gm = [&](int i) { if constexpr (CONSTTAB) return g0 ? P.gm0[i] : P.gmU[i]; else return __ldg(&T.Gm[s + i]); };
 
     // ---- load p_{s-1} .. p_{t_end}; the end nodes of the line are read as zero (R#7, R#8) ----
     cplx p[LC + 2];
@@ -59,7 +74,7 @@ k_sweep_xy(cplx* __restrict__ psi, LineMap map, SweepTables<CT> T, SweepFold fol
             cplx d = coef_mul(T.r, cadd(p[i], p[i + 2]));
             d = coef_fma(T.omr2, p[i + 1], d);
             d = coef_fma(T.r, e, d);
-            e = coef_mul(__ldg(&T.inv[s + i]), d);
+            e = coef_mul(t_inv(i), d);
             ev[i] = e;
         }
     }
@@ -74,8 +89,8 @@ k_sweep_xy(cplx* __restrict__ psi, LineMap map, SweepTables<CT> T, SweepFold fol
 #pragma unroll
         for (int i = LC - 1; i >= 0; --i) {
             if (i < cnt) {
-                const cplx ee = coef_fma(__ldg(&T.F[s + i]), ein, ev[i]);
-                x = csub(ee, coef_mul(__ldg(&T.cc[s + i]), x));
+                const cplx ee = coef_fma(t_F(i), ein, ev[i]);
+                x = csub(ee, coef_mul(t_cc(i), x));
                 ev[i] = x;
             }
         }
@@ -93,7 +108,7 @@ k_sweep_xy(cplx* __restrict__ psi, LineMap map, SweepTables<CT> T, SweepFold fol
 #pragma unroll
         for (int i = 0; i < LC; ++i) {
             if (i < cnt) {
-                const cplx v = coef_fma(__ldg(&T.Gm[s + i]), xin, ev[i]);
+                const cplx v = coef_fma(t_Gm(i), xin, ev[i]);
                 nrm += cabs2(v);
                 st_stream(gp + (long long)(s + i) * es, v);
             }

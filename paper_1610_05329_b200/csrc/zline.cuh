@@ -143,23 +143,13 @@ struct ZMainArgs {
     const cplx* tw;        // exp(-2 pi i j/M)
     const cplx* tws;       // exp(-2 pi i k/nz)
     double* phi_out;       // ZS_PHI
-};
-
-// Thomas tables of the z sweep as kernel parameters (constant bank: no load instruction at all), valid
-// when the elimination factors have converged by the second chunk (decided on the host, bitwise):
-// lane 0 uses chunk 0's entries, every other lane the converged chunk's.  (The forward inflow of lane 0
-// and the backward inflow of the last lane are zero, so F of chunk 0 and Gm of the last chunk never
-// matter.)  CONSTTAB = false reads the global tables instead (any r).
-template <typename CT, int LC>
-struct ZTabs {
-    CT inv0[LC], cc0[LC], gm0[LC];
-    CT invU[LC], ccU[LC], fU[LC], gmU[LC];
+    int pf_lines;          // L2 prefetch distance in lines (= lines resident on the GPU at a time); 0 = off
 };
 
 template <int NZ, typename CT, int SPEC, bool SWEEP, bool CONSTTAB, int WARPS, int MINB>
 __global__ void __launch_bounds__(32 * WARPS, MINB)
 k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, SweepTables<CT> T,
-         const __grid_constant__ ZTabs<CT, ZGeom<NZ>::LC> P)
+         const __grid_constant__ ChunkTabs<CT, ZGeom<NZ>::LC> P)
 {
     using G = ZGeom<NZ>;
     using PL = PosLine<NZ>;
@@ -176,6 +166,20 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
 
     // ---- stage the psi line and merge the half-spectrum; the global loads of both are issued before
     //      anything waits on them (psi in two batches to bound the registers in flight) ----
+    // ---- L2 prefetch for the warp that will run one residency later ----
+    if (Z.pf_lines > 0 && line + Z.pf_lines < Z.nlines) {
+        const char* pp = reinterpret_cast<const char*>(psi + (long long)(line + Z.pf_lines) * NZ);
+        if constexpr (USE_A) {
+#pragma unroll
+            for (int i = 0; i < (NZ * 16) / (128 * 32); ++i) prefetch_l2(pp + 128 * (lane + 32 * i));
+            if ((NZ * 16) % (128 * 32) != 0 && lane < ((NZ * 16) % (128 * 32)) / 128)
+                prefetch_l2(pp + 128 * (lane + 32 * ((NZ * 16) / (128 * 32))));
+        }
+        if constexpr (SPEC != ZS_NONE) {
+            const char* ps = reinterpret_cast<const char*>(spec + (long long)(line + Z.pf_lines) * (M + 1));
+            for (int o = 128 * lane; o < (M + 1) * 16; o += 128 * 32) prefetch_l2(ps + o);
+        }
+    }
     constexpr int HB = G::NPER / 2;
     cplx a[HB];
     if constexpr (USE_A) {
