@@ -4,7 +4,8 @@ updates/s at 512^3 on one B200; HBM GB/s vs peak).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--impl reference]
 
-One "step" = one pass of the whole hot path (kernels K1..K8) over the psi of the
+One "step" = one pass of the whole hot path (kernels K1..K8, the z sweep K8 fused into K5 when the z-line
+kernels apply) over the psi of the
 workload.  N = 1 times BASELINE.json's headline configuration C4 (512^3, imaginary time).  N > 1
 (torchrun, one rank per GPU) runs N independent replicas -- the path does not shard without all-to-all
 transposes -- and reports all ranks' steps over the slowest rank's time.
@@ -164,13 +165,17 @@ def run_reference(args, cfg):
 # the CUDA path
 # ------------------------------------------------------------------------------------------------
 def ncu_traffic(kernel_name):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, if one is recorded
-    in profiles/traffic.json ({kernel name: bytes}); else None."""
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from
+    the committed `ncu --set full` capture, recorded in profiles/traffic.csv; else None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(kernel_name)
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for line in f:
+                name, _, rest = line.rstrip("\n").partition(",")
+                if name == kernel_name:
+                    return float(rest.split(",")[0])
     except Exception:
-        return None
+        pass
+    return None
 
 
 def run_b200(args, cfg):
@@ -224,8 +229,14 @@ def run_b200(args, cfg):
                 "algorithmic_bytes_per_launch": top["bytes"], "kernel_ms": top["ms"],
                 "share_of_step": top["ms"] / sum(k["ms"] for k in kernels)}
     step_gbps = G.bytes_per_step / step_ms * 1e-6
+    built = sum(k["bytes"] for k in kernels)
     whole = {"algorithmic_bytes_per_step": G.bytes_per_step, "achieved": step_gbps, "frac": step_gbps / peak,
-             "unit": "GB/s", "model": "M1 = 144N + 8S (DESIGN.md section 7)"}
+             "unit": "GB/s", "model": "M1 = 144N + 8S (SURVEY section 8d; DESIGN.md section 7)",
+             "frac_of_nominal_8TBps": step_gbps / 8000.0,
+             "as_built": {"bytes_per_step": built, "achieved": built / step_ms * 1e-6,
+                          "frac": built / step_ms * 1e-6 / peak,
+                          "model": "sum of the kernels' own algorithmic bytes (M2 = 112N + 8S when the z sweep is "
+                                   "fused into K5)"}}
 
     # ---- end to end through the C-ABI with HOST buffers (dgpe_step_host) ----
     e2e = None
