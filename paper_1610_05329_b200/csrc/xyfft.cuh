@@ -101,7 +101,12 @@ k_fft_xy(cplx* __restrict__ data, LineMap map, const cplx* __restrict__ tw, UddA
             const bool origin_col = (ky == 0 && kz == 0);
             pf.modify(b, [&](int idx, cplx v) {
                 const double k2 = __ldg(&U.kx2[idx]) + qy + qz;
-                double u = FOUR_PI_3 * (3.0 * qz / k2 - 1.0);
+                // 1/k2 by two Newton steps from the single-precision reciprocal (<= 2 ulp; k2 is a sum of
+                // squared wave numbers, far inside the float range; k2 = 0 gives inf/NaN, replaced below)
+                double rk = (double)__frcp_rn((float)k2);
+                rk = rk * (2.0 - k2 * rk);
+                rk = rk * (2.0 - k2 * rk);
+                double u = FOUR_PI_3 * (3.0 * qz * rk - 1.0);
                 if (origin_col && idx == 0) u = 0.0;
                 u *= U.invN;
                 return mk(v.x * u, v.y * u);

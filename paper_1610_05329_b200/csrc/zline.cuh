@@ -182,6 +182,10 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
     }
     constexpr int HB = G::NPER / 2;
     cplx a[HB];
+    // Z_k, k = lane + 32 t, is exactly what butterfly `lane` of the first inverse pass reads when that pass
+    // has radix M/32: then the merged values go from registers straight into the pass
+    constexpr bool FIRST_IN_REGS = (SPEC != ZS_NONE) && (ct::radix_at(M, 0, false) == M / 32);
+    cplx xa[SPEC != ZS_NONE ? M / 32 : 1];
     if constexpr (USE_A) {
 #pragma unroll
         for (int i = 0; i < HB; ++i) a[i] = ld_stream(p + 32 * i + lane);
@@ -189,7 +193,7 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
     if constexpr (SPEC != ZS_NONE) {
         // Hermitian merge straight from global memory into the FFT buffer
         const cplx* in = spec + (long long)line * (M + 1);
-        cplx xa[M / 32], xb[M / 32];
+        cplx xb[M / 32];
 #pragma unroll
         for (int t = 0; t < M / 32; ++t) {
             const int k = lane + 32 * t;
@@ -209,7 +213,11 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
             const cplx cb = cconj(xb[t]);
             const cplx s = cadd(xa[t], cb), d = csub(xa[t], cb);
             const cplx wd = cmul(w, d);
-            B[PosPad::at(k)] = mk(s.x - wd.y, s.y + wd.x);        // s + i w d
+            xa[t] = mk(s.x - wd.y, s.y + wd.x);                   // Z_k = s + i w d
+        }
+        if constexpr (!FIRST_IN_REGS) {
+#pragma unroll
+            for (int t = 0; t < M / 32; ++t) B[PosPad::at(lane + 32 * t)] = xa[t];
         }
         if constexpr (USE_A) {
 #pragma unroll
@@ -230,7 +238,7 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         const double vxy = __ldg(&Z.vx[i]) + __ldg(&Z.vy[j]);
         const double s2 = Z.scal[SC_S2], s1 = Z.scal[SC_S1];
         auto none = [](int) { return mk(0.0, 0.0); };
-        ct_fft_range<M, true, false, 32, SyncWarp, PosPad, 0, L, false>(B, lane, true, Z.tw, none, [&](int m, cplx phi) {
+        auto nonlin = [&](int m, cplx phi) {
             if constexpr (SPEC == ZS_PHI) {
                 reinterpret_cast<double2*>(Z.phi_out + (long long)line * NZ)[m] = phi;
             } else {
@@ -253,7 +261,24 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
                     A[pos] = a;
                 }
             }
-        });
+        };
+        if constexpr (FIRST_IN_REGS) {
+            using P0 = CtPass<M, 0, true, false, 32>;
+            static_assert(P0::NB == 1 && P0::R == M / 32 && P0::Ns == 1, "first pass must be one butterfly per lane");
+            P0 p0;
+#pragma unroll
+            for (int q = 0; q < P0::R; ++q) p0.v[0][q] = xa[q];
+            p0.bfly(lane);
+            if constexpr (P0::LAST) {
+                p0.scatter(lane, nonlin);
+            } else {
+                p0.scatter(lane, [&](int idx, cplx val) { B[PosPad::at(idx)] = val; });
+                __syncwarp();
+                ct_fft_range<M, true, false, 32, SyncWarp, PosPad, 1, L, false>(B, lane, true, Z.tw, none, nonlin);
+            }
+        } else {
+            ct_fft_range<M, true, false, 32, SyncWarp, PosPad, 0, L, false>(B, lane, true, Z.tw, none, nonlin);
+        }
         __syncwarp();
     }
 
