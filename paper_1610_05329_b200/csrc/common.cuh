@@ -25,6 +25,8 @@ __device__ __forceinline__ double cabs2(cplx a) { return a.x * a.x + a.y * a.y; 
 // Coefficient arithmetic of the Crank-Nicolson tables: real in imaginary time, complex in real time.
 __device__ __forceinline__ cplx coef_mul(double c, cplx v) { return mk(c * v.x, c * v.y); }
 __device__ __forceinline__ cplx coef_mul(cplx c, cplx v) { return cmul(c, v); }
+__device__ __forceinline__ double coef_neg(double c) { return -c; }
+__device__ __forceinline__ cplx coef_neg(cplx c) { return mk(-c.x, -c.y); }
 // a + c*b
 __device__ __forceinline__ cplx coef_fma(double c, cplx b, cplx a) { return mk(fma(c, b.x, a.x), fma(c, b.y, a.y)); }
 __device__ __forceinline__ cplx coef_fma(cplx c, cplx b, cplx a)

@@ -71,10 +71,11 @@ k_sweep_xy(cplx* __restrict__ psi, LineMap map, SweepTables<CT> T, SweepFold fol
     for (int i = 0; i < LC; ++i) {
         ev[i] = mk(0.0, 0.0);
         if (work && i < cnt) {
+            // e_j = inv_j (d_j + r e_{j-1}) written as inv_j d_j + (r inv_j) e_{j-1}, r inv_j = -c_j: one
+            // dependent fma per unknown instead of an fma and a multiply
             cplx d = coef_mul(T.r, cadd(p[i], p[i + 2]));
             d = coef_fma(T.omr2, p[i + 1], d);
-            d = coef_fma(T.r, e, d);
-            e = coef_mul(t_inv(i), d);
+            e = coef_fma(coef_neg(t_cc(i)), e, coef_mul(t_inv(i), d));
             ev[i] = e;
         }
     }
@@ -90,7 +91,7 @@ k_sweep_xy(cplx* __restrict__ psi, LineMap map, SweepTables<CT> T, SweepFold fol
         for (int i = LC - 1; i >= 0; --i) {
             if (i < cnt) {
                 const cplx ee = coef_fma(t_F(i), ein, ev[i]);
-                x = csub(ee, coef_mul(t_cc(i), x));
+                x = coef_fma(coef_neg(t_cc(i)), x, ee);
                 ev[i] = x;
             }
         }

@@ -307,10 +307,10 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
                 if (i < cnt) {
                     const int jn = s + i + 1;
                     const cplx pp = (jn < NZ - 1) ? A[PL::at(jn)] : mk(0.0, 0.0);
+                    // inv_j (d_j + r e_{j-1}) = inv_j d_j + (-c_j) e_{j-1}: one dependent fma per unknown
                     cplx d = coef_mul(T.r, cadd(pm, pp));
                     d = coef_fma(T.omr2, p0, d);
-                    d = coef_fma(T.r, e, d);
-                    e = coef_mul(t_inv(i), d);
+                    e = coef_fma(coef_neg(t_cc(i)), e, coef_mul(t_inv(i), d));
                     ev[i] = e;
                     pm = p0;
                     p0 = pp;
@@ -333,7 +333,7 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         for (int i = LC - 1; i >= 0; --i) {
             if (i < cnt) {
                 const cplx ee = coef_fma(t_F(i), ein, ev[i]);
-                x = csub(ee, coef_mul(t_cc(i), x));
+                x = coef_fma(coef_neg(t_cc(i)), x, ee);
                 ev[i] = x;
             }
         }
