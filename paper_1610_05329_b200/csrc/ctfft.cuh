@@ -66,10 +66,33 @@ struct CtPass {
     static constexpr bool LAST = (P == NPASS - 1);
 
     cplx v[NB][R];
+    cplx w[Ns > 1 ? NB : 1][R];      // twiddles w^q of this slot's butterflies (unused when Ns == 1)
 
-    // v_q = f(j + q N/R) for this slot's butterflies, then the twiddles (tw[m] = exp(-2 pi i m/N))
+    // Twiddles w^q, w = tw[k TWSTEP] (tw[m] = exp(-2 pi i m/N)): the powers 1, 2, 4 come from the fp64
+    // table, the others are one product of two table entries (<= 3 ulp), which trades 4 of the 7 table
+    // loads of a radix-8 butterfly for 4 complex multiplications.  Independent of the data, so callers
+    // issue it BEFORE the barrier that guards the data: the table loads overlap the barrier wait.
+    __device__ __forceinline__ void load_tw(int b, const cplx* __restrict__ tw)
+    {
+        if constexpr (Ns > 1) {
+#pragma unroll
+            for (int u = 0; u < NB; ++u) {
+                const int j = b + u * NBF;
+                if (EXACT || j < NBUT) {
+                    const int k = j % Ns;
+#pragma unroll
+                    for (int q = 1; q < R; q <<= 1) {
+                        w[u][q] = __ldg(&tw[q * k * TWSTEP]);
+                        if (INV) w[u][q].y = -w[u][q].y;
+                    }
+                }
+            }
+        }
+    }
+
+    // v_q = f(j + q N/R) w^q for this slot's butterflies (load_tw first)
     template <class F>
-    __device__ __forceinline__ void load(int b, const cplx* __restrict__ tw, F&& f)
+    __device__ __forceinline__ void load(int b, F&& f)
     {
 #pragma unroll
         for (int u = 0; u < NB; ++u) {
@@ -77,25 +100,15 @@ struct CtPass {
             if (EXACT || j < NBUT) {
 #pragma unroll
                 for (int q = 0; q < R; ++q) v[u][q] = f(j + q * NBUT);
-                if (Ns > 1) {
-                    // twiddles w^q, w = tw[k TWSTEP]: the powers 1, 2, 4 come from the fp64 table, the
-                    // others are one product of two table entries (<= 3 ulp), which trades 4 of the 7
-                    // table loads of a radix-8 butterfly for 4 complex multiplications
-                    const int k = j % Ns;
-                    cplx w[R];
-#pragma unroll
-                    for (int q = 1; q < R; q <<= 1) {
-                        w[q] = __ldg(&tw[q * k * TWSTEP]);
-                        if (INV) w[q].y = -w[q].y;
-                    }
-                    if (R >= 4) w[3] = cmul(w[1], w[2]);
+                if constexpr (Ns > 1) {
+                    if (R >= 4) w[u][3] = cmul(w[u][1], w[u][2]);
                     if (R == 8) {
-                        w[5] = cmul(w[1], w[4]);
-                        w[6] = cmul(w[2], w[4]);
-                        w[7] = cmul(w[3], w[4]);
+                        w[u][5] = cmul(w[u][1], w[u][4]);
+                        w[u][6] = cmul(w[u][2], w[u][4]);
+                        w[u][7] = cmul(w[u][3], w[u][4]);
                     }
 #pragma unroll
-                    for (int q = 1; q < R; ++q) v[u][q] = cmul(v[u][q], w[q]);
+                    for (int q = 1; q < R; ++q) v[u][q] = cmul(v[u][q], w[u][q]);
                 }
             }
         }
@@ -152,27 +165,43 @@ struct SyncWarp { static __device__ __forceinline__ void sync() { __syncwarp(); 
 // `on` = this thread owns butterfly slot b (threads that do not still take part in the barriers).
 // When FROM_F is false the caller must have synchronised the team after the column was written; when
 // it is true the column must be free to overwrite.
+// worker: the twiddles of pass P are already in `pass` (loaded before the preceding barrier)
+template <int N, bool INV, bool REV, int NBF, class Sync, class Pos, int P, int PEND, bool FROM_F, class FFirst,
+          class FLast>
+__device__ __forceinline__ void ct_fft_range_tw(CtPass<N, P, INV, REV, NBF>& pass, cplx* col, int b, bool on,
+                                                const cplx* __restrict__ tw, FFirst&& first, FLast&& last)
+{
+    using Pass = CtPass<N, P, INV, REV, NBF>;
+    if (on) {
+        if constexpr (FROM_F) pass.load(b, first);
+        else pass.load(b, [&](int idx) { return col[Pos::at(idx)]; });
+    }
+    if constexpr (!FROM_F) Sync::sync();          // every read of this pass precedes its writes
+    if (on) pass.bfly(b);
+    if constexpr (Pass::LAST) {
+        if (on) pass.scatter(b, last);
+    } else {
+        if (on) pass.scatter(b, [&](int idx, cplx val) { col[Pos::at(idx)] = val; });
+        if constexpr (P + 1 < PEND) {
+            CtPass<N, P + 1, INV, REV, NBF> next;
+            if (on) next.load_tw(b, tw);          // overlaps the barrier wait
+            Sync::sync();
+            ct_fft_range_tw<N, INV, REV, NBF, Sync, Pos, P + 1, PEND, false>(next, col, b, on, tw, first, last);
+        } else {
+            Sync::sync();
+        }
+    }
+}
+
 template <int N, bool INV, bool REV, int NBF, class Sync, class Pos, int P, int PEND, bool FROM_F, class FFirst,
           class FLast>
 __device__ __forceinline__ void ct_fft_range(cplx* col, int b, bool on, const cplx* __restrict__ tw, FFirst&& first,
                                              FLast&& last)
 {
     if constexpr (P < PEND) {
-        using Pass = CtPass<N, P, INV, REV, NBF>;
-        Pass pass;
-        if (on) {
-            if constexpr (FROM_F) pass.load(b, tw, first);
-            else pass.load(b, tw, [&](int idx) { return col[Pos::at(idx)]; });
-        }
-        if constexpr (!FROM_F) Sync::sync();          // every read of this pass precedes its writes
-        if (on) pass.bfly(b);
-        if constexpr (Pass::LAST) {
-            if (on) pass.scatter(b, last);
-        } else {
-            if (on) pass.scatter(b, [&](int idx, cplx val) { col[Pos::at(idx)] = val; });
-            Sync::sync();
-            ct_fft_range<N, INV, REV, NBF, Sync, Pos, P + 1, PEND, false>(col, b, on, tw, first, last);
-        }
+        CtPass<N, P, INV, REV, NBF> pass;
+        if (on) pass.load_tw(b, tw);
+        ct_fft_range_tw<N, INV, REV, NBF, Sync, Pos, P, PEND, FROM_F>(pass, col, b, on, tw, first, last);
     }
 }
 

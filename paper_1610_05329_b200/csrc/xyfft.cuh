@@ -87,8 +87,9 @@ k_fft_xy(cplx* __restrict__ data, LineMap map, const cplx* __restrict__ tw, UddA
         static_assert(PF::R == PI::R && PF::NB == PI::NB && PI::Ns == 1, "forward-last and inverse-first passes must match");
         PF pf;
         if (on) {
-            if constexpr (L == 1) pf.load(b, tw, from_g);
-            else pf.load(b, tw, [&](int idx) { return colsm[PosTile::at(idx)]; });
+            pf.load_tw(b, tw);
+            if constexpr (L == 1) pf.load(b, from_g);
+            else pf.load(b, [&](int idx) { return colsm[PosTile::at(idx)]; });
         }
         if constexpr (L > 1) __syncthreads();
         PI pi;
