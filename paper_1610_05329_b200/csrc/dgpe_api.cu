@@ -91,6 +91,13 @@ struct dgpe_handle {
     double* d_out = nullptr;         // device results (16 doubles)
     double* h_out = nullptr;         // pinned host mirror
     cplx* psi_stage = nullptr;       // dgpe_step_host: device copy of psi (lazy)
+    // CUDA graph of one step (7 or 8 kernel nodes), captured once per psi pointer on a private stream and
+    // replayed on the handle's stream: removes the per-launch host cost that dominates the small grids
+    bool use_graph = true;           // DGPE_GRAPH=0: plain launches
+    bool warmed = false;             // one eager step has run (lazy per-kernel attribute setup done)
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t step_exec = nullptr;
+    cplx* step_exec_psi = nullptr;
     std::vector<cudaEvent_t> prof_ev; // dgpe_step_profile
     std::vector<void*> owned;        // everything to cudaFree
 };
@@ -286,6 +293,8 @@ static int init_handle(dgpe_handle* h)
         h->zfast = !h->force_generic && z_specialised(nz);
         const char* pf = getenv("DGPE_PREFETCH");
         if (pf && pf[0]) h->prefetch = atoi(pf);
+        const char* gr = getenv("DGPE_GRAPH");
+        h->use_graph = !(gr && gr[0] == '0');
         const char* pm = getenv("DGPE_PF_MULT");
         if (pm && atoi(pm) > 0) h->pf_mult = atoi(pm);
     }
@@ -418,6 +427,8 @@ extern "C" void dgpe_destroy(dgpe_handle* h)
 {
     if (!h) return;
     cudaStreamSynchronize(h->stream);
+    if (h->step_exec) cudaGraphExecDestroy(h->step_exec);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     for (void* p : h->owned) cudaFree(p);
     if (h->h_out) cudaFreeHost(h->h_out);
     for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
@@ -834,6 +845,45 @@ static int check_finite(dgpe_handle* h)
     return DGPE_OK;
 }
 
+// nsteps steps on the handle's stream: the first ever step eagerly (it also finishes the lazy kernel
+// attribute setup), the others as replays of the captured one-step graph.
+static int run_steps(dgpe_handle* h, cplx* psi, int nsteps)
+{
+    int rc, s = 0;
+    if (!h->warmed && nsteps > 0) {
+        if ((rc = one_step(h, psi, [](int) {}))) return rc;
+        h->warmed = true;
+        s = 1;
+    }
+    if (h->use_graph && nsteps - s >= 2) {
+        if (!h->step_exec || h->step_exec_psi != psi) {
+            if (h->step_exec) { cudaGraphExecDestroy(h->step_exec); h->step_exec = nullptr; }
+            if (!h->cap_stream) CU(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+            cudaStream_t user = h->stream;
+            h->stream = h->cap_stream;
+            cudaGraph_t graph = nullptr;
+            cudaError_t e = cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal);
+            rc = (e == cudaSuccess) ? one_step(h, psi, [](int) {}) : DGPE_ERR_CUDA;
+            cudaError_t e2 = (e == cudaSuccess) ? cudaStreamEndCapture(h->cap_stream, &graph) : e;
+            h->stream = user;
+            if (rc || e2 != cudaSuccess || !graph) {
+                if (graph) cudaGraphDestroy(graph);
+                cudaGetLastError();
+                return fail(DGPE_ERR_CUDA, "capturing the step graph failed: %s", cudaGetErrorString(e2));
+            }
+            e = cudaGraphInstantiate(&h->step_exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) { h->step_exec = nullptr; return fail(DGPE_ERR_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e)); }
+            h->step_exec_psi = psi;
+        }
+        for (; s < nsteps; ++s) CU(cudaGraphLaunch(h->step_exec, h->stream));
+        return DGPE_OK;
+    }
+    for (; s < nsteps; ++s)
+        if ((rc = one_step(h, psi, [](int) {}))) return rc;
+    return DGPE_OK;
+}
+
 extern "C" int dgpe_step(dgpe_handle* h, void* psi_, int nsteps)
 {
     if (!h || !psi_) return fail(DGPE_ERR_ARG, "NULL handle or psi");
@@ -842,8 +892,7 @@ extern "C" int dgpe_step(dgpe_handle* h, void* psi_, int nsteps)
     cplx* psi = (cplx*)psi_;
     int rc;
     if ((rc = set_scal(h, 1))) return rc;
-    for (int s = 0; s < nsteps; ++s)
-        if ((rc = one_step(h, psi, [](int) {}))) return rc;
+    if ((rc = run_steps(h, psi, nsteps))) return rc;
     if (h->mode == DGPE_IMAG) {
         if ((rc = finish_steps(h, psi))) return rc;
         CU(cudaStreamSynchronize(h->stream));
@@ -866,8 +915,7 @@ extern "C" int dgpe_step_host(dgpe_handle* h, void* psi_host, int nsteps)
     bool imag_done = false;
     if (nsteps > 0) {
         if ((rc = set_scal(h, 1))) return rc;
-        for (int s = 0; s < nsteps; ++s)
-            if ((rc = one_step(h, h->psi_stage, [](int) {}))) return rc;
+        if ((rc = run_steps(h, h->psi_stage, nsteps))) return rc;
         if (h->mode == DGPE_IMAG) {
             if ((rc = finish_steps(h, h->psi_stage))) return rc;
             imag_done = true;
