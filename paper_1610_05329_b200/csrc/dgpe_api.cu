@@ -12,6 +12,8 @@
 #include <cstring>
 #include <vector>
 
+#include <cudaTypedefs.h>
+
 #include "common.cuh"
 #include "fft.cuh"
 #include "observe.cuh"
@@ -19,6 +21,7 @@
 #include "sweep.cuh"
 #include "xyfft.cuh"
 #include "xysweep.cuh"
+#include "xysweep_tma.cuh"
 #include "zline.cuh"
 
 using namespace dgpe;
@@ -76,6 +79,8 @@ struct dgpe_handle {
     // L2 prefetch of the next residency, per kernel family (DGPE_PREFETCH=<mask> overrides, for A/B runs):
     // it pays for the z-line kernels and the y axis; on the x axis (row stride ny*nz) it costs time
     int prefetch = PF_Z | PF_SWEEP_Y | PF_FFT_Y;
+    bool use_tma_x = false;          // DGPE_TMA=2: TMA on the x axis at every length (A/B)
+    bool use_tma = true;             // DGPE_TMA=0: the x/y sweeps load and store through the threads (k_sweep_xy)
     bool zfast = false;              // warp-per-line z kernels (zline.cuh) and the fused step order z, x, y
 
     cplx* spec = nullptr;                       // [nx][ny][nzh]
@@ -293,6 +298,9 @@ static int init_handle(dgpe_handle* h)
         h->zfast = !h->force_generic && z_specialised(nz);
         const char* pf = getenv("DGPE_PREFETCH");
         if (pf && pf[0]) h->prefetch = atoi(pf);
+        const char* tm = getenv("DGPE_TMA");
+        h->use_tma = !(tm && tm[0] == '0');
+        h->use_tma_x = tm && tm[0] == '2';
         const char* gr = getenv("DGPE_GRAPH");
         h->use_graph = !(gr && gr[0] == '0');
         const char* pm = getenv("DGPE_PF_MULT");
@@ -336,7 +344,7 @@ static int init_handle(dgpe_handle* h)
         const double rr = h->dt / (4.0 * ds[a] * ds[a]);      // R#9
         // chunk length of the sweep recursions: 8 (or 16) unknowns per thread on the strided axes; on z
         // the warp-per-line kernel gives every lane ceil((nz-2)/32) unknowns
-        int lc = (ns[a] <= 514 && !h->force_generic) ? 8 : 16;
+        int lc = (ns[a] <= 770 && !h->force_generic) ? 8 : 16;
         if (a == 2 && h->zfast) lc = (nz - 2 + 31) / 32;
         if (h->mode == DGPE_IMAG)
             rc = build_sweep<double>(h, &h->sw[a], ns[a], std::complex<double>(rr, 0.0), lc);
@@ -723,11 +731,96 @@ static int launch_c2r(dgpe_handle* h, cplx* psi, int kmode, double* out)
     return check_launch("k_c2r_nonlin");
 }
 
-template <typename CT, int LC, bool CONSTTAB, int MINB>
+// ---- TMA-fed persistent sweep (xysweep_tma.cuh) ----
+static PFN_cuTensorMapEncodeTiled_v12000 tensor_map_encoder()
+{
+    static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (PFN_cuTensorMapEncodeTiled_v12000)p;
+        cudaGetLastError();
+    }
+    return fn;
+}
+
+// can the TMA kernel take this sweep?  (whole tiles, a tile stage count >= 2 in shared memory, boxes <= 256 rows)
+static bool tma_sweep_ok(const dgpe_handle* h, const LineMap& m, const AxisSweep& S, int* box_rows, int* nstage)
+{
+    if (!h->use_tma || h->force_generic || S.Lc != TMA_LC || S.G > 96 || m.ncols % TILE_COLS) return false;
+    if (!tensor_map_encoder()) return false;
+    const int nbox = (m.n + 255) / 256;
+    if (m.n % nbox) return false;
+    const size_t tile = (size_t)m.n * TILE_COLS * sizeof(cplx);
+    int ns = (int)((200 * 1024) / tile);
+    if (ns < 2) return false;
+    // three stages when only one CTA fits on an SM anyway (tiles of 64 KB); two stages and several CTAs
+    // per SM for the short lines, whose CTAs are small
+    *nstage = (ns >= 3 && tile > 40 * 1024) ? 3 : 2;
+    if (const char* e = getenv("DGPE_TMA_STAGES")) { const int v = atoi(e); if (v >= 2 && v <= ns && v <= 3) *nstage = v; }
+    *box_rows = m.n / nbox;
+    return true;
+}
+
+template <typename CT, bool CONSTTAB, int NSTAGE, int NTMAX>
+static int launch_sweep_tma_s(dgpe_handle* h, cplx* psi, int axis, const LineMap& m, int box_rows, int thr,
+                              const SweepTables<CT>& T, const SweepFold& F, const AxisSweep& S)
+{
+    auto kern = k_sweep_tma<CT, CONSTTAB, NSTAGE, NTMAX>;
+    const size_t smem = (size_t)NSTAGE * m.n * TILE_COLS * sizeof(cplx) + 128;
+    static size_t allowed = 0;
+    if (smem > allowed) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        allowed = smem;
+    }
+    int ctas_per_sm = 1;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, thr, smem));
+    if (ctas_per_sm < 1) return fail(DGPE_ERR_CUDA, "k_sweep_tma does not fit on an SM (n = %d)", m.n);
+    // psi viewed as doubles: x sweep {2 ny nz, nx, 1}, y sweep {2 nz, ny, nx}; box {16, box_rows, 1}
+    const cuuint64_t nx = h->nx, ny = h->ny, nz = h->nz;
+    cuuint64_t dims[3], strides[2];
+    if (axis == 0) { dims[0] = 2 * ny * nz; dims[1] = nx; dims[2] = 1; strides[0] = ny * nz * 16; strides[1] = nx * ny * nz * 16; }
+    else { dims[0] = 2 * nz; dims[1] = ny; dims[2] = nx; strides[0] = nz * 16; strides[1] = ny * nz * 16; }
+    cuuint32_t box[3] = {2 * TILE_COLS, (cuuint32_t)box_rows, 1}, estr[3] = {1, 1, 1};
+    CUtensorMap tmap;
+    CUresult cr = tensor_map_encoder()(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, psi, dims, strides, box, estr,
+                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                       CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (cr != CUDA_SUCCESS) return fail(DGPE_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)cr);
+    TmaWalk W;
+    W.n = m.n; W.box_rows = box_rows;
+    W.tiles_per_batch = m.ncols / TILE_COLS;
+    W.ntiles = W.tiles_per_batch * (axis == 0 ? 1 : h->nx);
+    ChunkTabs<CT, TMA_LC> P;
+    fill_chunk_tabs<CT, TMA_LC>(S, CONSTTAB, &P);
+    const int grid = std::min(W.ntiles, h->num_sms * ctas_per_sm);
+    kern<<<grid, thr, smem, h->stream>>>(tmap, W, T, F, P);
+    return check_launch("k_sweep_tma");
+}
+
+template <typename CT, bool CONSTTAB>
+static int launch_sweep_tma(dgpe_handle* h, cplx* psi, int axis, const LineMap& m, int box_rows, int nstage, int thr,
+                            const SweepTables<CT>& T, const SweepFold& F, const AxisSweep& S)
+{
+    if (thr <= 256)
+        return nstage == 2 ? launch_sweep_tma_s<CT, CONSTTAB, 2, 256>(h, psi, axis, m, box_rows, thr, T, F, S)
+                           : launch_sweep_tma_s<CT, CONSTTAB, 3, 256>(h, psi, axis, m, box_rows, thr, T, F, S);
+    if (thr <= 512)
+        return nstage == 2 ? launch_sweep_tma_s<CT, CONSTTAB, 2, 512>(h, psi, axis, m, box_rows, thr, T, F, S)
+                           : launch_sweep_tma_s<CT, CONSTTAB, 3, 512>(h, psi, axis, m, box_rows, thr, T, F, S);
+    return nstage == 2 ? launch_sweep_tma_s<CT, CONSTTAB, 2, 768>(h, psi, axis, m, box_rows, thr, T, F, S)
+                       : launch_sweep_tma_s<CT, CONSTTAB, 3, 768>(h, psi, axis, m, box_rows, thr, T, F, S);
+}
+
+template <typename CT, int LC, bool CONSTTAB, int NTMAX, int MINB>
 static int launch_sweep_xy(dgpe_handle* h, cplx* psi, const LineMap& m, dim3 grid, int thr, const SweepTables<CT>& T,
                            const SweepFold& F, const AxisSweep& S)
 {
-    auto kern = k_sweep_xy<CT, LC, CONSTTAB, 512, MINB>;
+    auto kern = k_sweep_xy<CT, LC, CONSTTAB, NTMAX, MINB>;
     ChunkTabs<CT, LC> P;
     fill_chunk_tabs<CT, LC>(S, CONSTTAB, &P);
     int ctas_per_sm = 0;
@@ -753,13 +846,27 @@ static int launch_sweep_t(dgpe_handle* h, cplx* psi, int axis, bool fold)
     F.dV = h->dx * h->dy * h->dz;
     F.partials = h->partials; F.ticket = h->ticket; F.scal = h->scal;
     const int thr = threads_for(S.G);
-    if (axis < 2 && !h->force_generic && S.G <= 64 && (S.Lc == 8 || S.Lc == 16)) {
+    if (axis < 2 && !h->force_generic) {
         LineMap m = axis == 0 ? LineMap{nx, ny * nz, 0, 1, (long long)ny * nz} : LineMap{ny, nz, (long long)ny * nz, 1, nz};
+        int box_rows = 0, nstage = 0;
+        // Where the TMA pipeline pays (measured): the y axis from n = 384 up (512^3:
+        // 0.75 vs 0.83 ms) and both axes for the long lines whose thread-loading CTAs are few and large
+        // (768: 1.7 vs 2.3 ms).  On the x axis at n = 512 (rows ny*nz*16 bytes apart, one page each) it is
+        // slower (0.94 vs 0.83 ms), and so it is for the short lines (256^3: 0.19 vs 0.11 ms).
+        const bool want_tma = (axis == 1 && m.n >= 384) || S.G > 64 || (h->use_tma_x);
+        if (want_tma && tma_sweep_ok(h, m, S, &box_rows, &nstage))
+            return S.consttab ? launch_sweep_tma<CT, true>(h, psi, axis, m, box_rows, nstage, thr, T, F, S)
+                              : launch_sweep_tma<CT, false>(h, psi, axis, m, box_rows, nstage, thr, T, F, S);
         dim3 grid((m.ncols + TILE_COLS - 1) / TILE_COLS, axis == 0 ? 1 : nx);
-        if (S.Lc == 8) return S.consttab ? launch_sweep_xy<CT, 8, true, 2>(h, psi, m, grid, thr, T, F, S)
-                                         : launch_sweep_xy<CT, 8, false, 2>(h, psi, m, grid, thr, T, F, S);
-        return S.consttab ? launch_sweep_xy<CT, 16, true, 1>(h, psi, m, grid, thr, T, F, S)
-                          : launch_sweep_xy<CT, 16, false, 1>(h, psi, m, grid, thr, T, F, S);
+        if (S.Lc == 8 && S.G <= 64)
+            return S.consttab ? launch_sweep_xy<CT, 8, true, 512, 2>(h, psi, m, grid, thr, T, F, S)
+                              : launch_sweep_xy<CT, 8, false, 512, 2>(h, psi, m, grid, thr, T, F, S);
+        if (S.Lc == 8 && S.G <= 96)
+            return S.consttab ? launch_sweep_xy<CT, 8, true, 768, 1>(h, psi, m, grid, thr, T, F, S)
+                              : launch_sweep_xy<CT, 8, false, 768, 1>(h, psi, m, grid, thr, T, F, S);
+        if (S.Lc == 16 && S.G <= 64)
+            return S.consttab ? launch_sweep_xy<CT, 16, true, 512, 1>(h, psi, m, grid, thr, T, F, S)
+                              : launch_sweep_xy<CT, 16, false, 512, 1>(h, psi, m, grid, thr, T, F, S);
     }
     if (axis == 0) {
         LineMap m{nx, ny * nz, 0, 1, (long long)ny * nz};
