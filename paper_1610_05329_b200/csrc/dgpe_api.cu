@@ -345,7 +345,7 @@ static int init_handle(dgpe_handle* h)
         // chunk length of the sweep recursions: 8 (or 16) unknowns per thread on the strided axes; on z
         // the warp-per-line kernel gives every lane ceil((nz-2)/32) unknowns
         int lc = (ns[a] <= 770 && !h->force_generic) ? 8 : 16;
-        if (a == 2 && h->zfast) lc = (nz - 2 + 31) / 32;
+        if (a == 2 && h->zfast) lc = ((nz - 2 + 31) / 32) | 1;      // odd: conflict-free chunk walks (zline.cuh)
         if (h->mode == DGPE_IMAG)
             rc = build_sweep<double>(h, &h->sw[a], ns[a], std::complex<double>(rr, 0.0), lc);
         else
@@ -548,7 +548,8 @@ static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
     ZMainArgs Z;
     Z.nlines = h->nx * h->ny; Z.ny = h->ny;
     Z.dt = h->dt; Z.g = h->g; Z.gdd = h->gdd;
-    Z.vx = h->vx; Z.vy = h->vy; Z.vz = h->vz;
+    Z.vx = h->vx; Z.vy = h->vy;
+    Z.dz = h->dz; Z.lam2 = h->lambda * h->lambda;
     Z.scal = h->scal; Z.tw = h->tw_zh; Z.tws = h->tw_split; Z.phi_out = phi_out;
     {
         static int ctas_per_sm = 0;

@@ -16,45 +16,31 @@
 //
 // Shared memory per warp:
 //   B  FFT buffer, M = nz/2 complex, element idx at idx + (idx >> 3)  (the one pad per 8 elements makes
-//      the stride-R writes of the first pass conflict free);
-//   A  the psi line, even and odd elements in two padded halves (PosLine): the coalesced walks along the
-//      line, the pair walk of the nonlinear update and the per-lane walks along a sweep chunk are all
-//      conflict free.
+//      the stride-R writes of the first pass conflict free); the last inverse pass leaves Phi in it as
+//      nz plain doubles;
+//   A  the psi line, nz complex, LINEAR: it arrives by ONE bulk asynchronous copy (cp.async.bulk, the TMA
+//      engine, completion on an mbarrier) and leaves by one bulk store, so no thread issues a global load
+//      or store for psi.  Lane l owns the LC unknowns 1 + l LC .. of the line; LC is ODD (17 at nz = 512),
+//      so the per-lane walks along the chunks are free of bank conflicts without any padding.
 #pragma once
 #include "ctfft.cuh"
 #include "sweep.cuh"
+#include "tma.cuh"
 
 namespace dgpe {
 
 template <int NZ>
 struct ZGeom {
     static constexpr int M = NZ / 2;
-    static constexpr int NPER = NZ / 32;                 // psi elements per lane
-    static constexpr int LC = (NZ - 2 + 31) / 32;        // sweep chunk per lane
-    static constexpr int HALF = ((M + (M >> 3) + 7) / 8) * 8 + 4;      // offset of the odd half, = 4 mod 8
-    static constexpr int A_ELEMS = (HALF + M + (M >> 3) + 7) / 8 * 8;
+    static constexpr int NPER = NZ / 32;                       // psi elements per lane (coalesced walks)
+    static constexpr int LC = ((NZ - 2 + 31) / 32) | 1;        // sweep chunk per lane, odd
+    static constexpr int A_ELEMS = NZ;
     static constexpr int B_ELEMS = (M + (M >> 3) + 7) / 8 * 8;
     static_assert(NZ % 64 == 0, "z-line kernels need nz to be a multiple of 64");
-    static_assert(LC % 2 == 0, "the chunk walk is conflict free only for an even chunk length");
 };
 
 struct PosPad {
     static __device__ __forceinline__ int at(int idx) { return idx + (idx >> 3); }
-};
-
-// Line buffer A: element e = 2m + t lives at t*HALF + m + (m >> 3).  Three access patterns are all
-// free of bank conflicts (16-byte elements: the 8 lanes of a quarter-warp must hit 8 different
-// positions mod 8):  the coalesced walk (lane <-> e), 4 even and 4 odd elements per quarter-warp, the
-// halves 4 banks apart;  the pair walk of the nonlinear update (lane <-> m);  the chunk walk of the
-// sweep (lane <-> e = 1 + LC lane + i, LC even: m advances by LC/2 per lane, the pad makes the stride odd
-// for LC = 16).
-template <int NZ>
-struct PosLine {
-    static __device__ __forceinline__ int at(int e)
-    {
-        const int m = e >> 1;
-        return (e & 1) * ZGeom<NZ>::HALF + m + (m >> 3);
-    }
 };
 
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
@@ -138,7 +124,8 @@ enum { ZS_NONE = 0, ZS_IMAG = 1, ZS_REAL = 2, ZS_PHI = 3 };
 struct ZMainArgs {
     int nlines, ny;
     double dt, g, gdd;
-    const double *vx, *vy, *vz;
+    double dz, lam2;       // z_k = (k - nz/2) dz, V_z = lambda^2 z_k^2 / 2 (evaluated in the kernel, no table walk)
+    const double *vx, *vy;
     const double* scal;
     const cplx* tw;        // exp(-2 pi i j/M)
     const cplx* tws;       // exp(-2 pi i k/nz)
@@ -146,16 +133,32 @@ struct ZMainArgs {
     int pf_lines;          // L2 prefetch distance in lines (= lines resident on the GPU at a time); 0 = off
 };
 
+// one bulk asynchronous copy global -> shared (TMA engine), completion counted on an mbarrier
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gsrc, unsigned bytes, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(
+                     smem_addr(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_addr(bar))
+                 : "memory");
+}
+// one bulk asynchronous copy shared -> global, tracked by the issuing thread's bulk async-groups
+__device__ __forceinline__ void bulk_store(void* gdst, const void* smem_src, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n" ::"l"(gdst), "r"(smem_addr(smem_src)),
+                 "r"(bytes)
+                 : "memory");
+}
+
 template <int NZ, typename CT, int SPEC, bool SWEEP, bool CONSTTAB, int WARPS, int MINB>
 __global__ void __launch_bounds__(32 * WARPS, MINB)
 k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, SweepTables<CT> T,
          const __grid_constant__ ChunkTabs<CT, ZGeom<NZ>::LC> P)
 {
     using G = ZGeom<NZ>;
-    using PL = PosLine<NZ>;
     constexpr int M = G::M, L = ct::npass(M), LC = G::LC;
     constexpr bool USE_A = (SPEC != ZS_PHI);
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ __align__(8) unsigned long long bars[WARPS];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int line = blockIdx.x * WARPS + warp;
     if (line >= Z.nlines) return;                       // warps are independent: no block barrier below
@@ -164,47 +167,39 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
     cplx* B = A + (USE_A ? G::A_ELEMS : 0);
     cplx* p = psi + (long long)line * NZ;
 
-    // ---- stage the psi line and merge the half-spectrum; the global loads of both are issued before
-    //      anything waits on them (psi in two batches to bound the registers in flight) ----
+    // ---- the psi line: one bulk copy, in flight while the spectrum is loaded, merged and transformed ----
+    if constexpr (USE_A) {
+        if (lane == 0) {
+            mbar_init(&bars[warp], 1);
+            mbar_fence_init();
+            mbar_expect_tx(&bars[warp], NZ * 16u);
+            bulk_load(A, p, NZ * 16u, &bars[warp]);
+        }
+    }
     // ---- L2 prefetch for the warp that will run one residency later ----
     if (Z.pf_lines > 0 && line + Z.pf_lines < Z.nlines) {
         const char* pp = reinterpret_cast<const char*>(psi + (long long)(line + Z.pf_lines) * NZ);
         if constexpr (USE_A) {
-#pragma unroll
-            for (int i = 0; i < (NZ * 16) / (128 * 32); ++i) prefetch_l2(pp + 128 * (lane + 32 * i));
-            if ((NZ * 16) % (128 * 32) != 0 && lane < ((NZ * 16) % (128 * 32)) / 128)
-                prefetch_l2(pp + 128 * (lane + 32 * ((NZ * 16) / (128 * 32))));
+            for (int o = 128 * lane; o < NZ * 16; o += 128 * 32) prefetch_l2(pp + o);
         }
         if constexpr (SPEC != ZS_NONE) {
             const char* ps = reinterpret_cast<const char*>(spec + (long long)(line + Z.pf_lines) * (M + 1));
             for (int o = 128 * lane; o < (M + 1) * 16; o += 128 * 32) prefetch_l2(ps + o);
         }
     }
-    constexpr int HB = G::NPER / 2;
-    cplx a[HB];
-    // Z_k, k = lane + 32 t, is exactly what butterfly `lane` of the first inverse pass reads when that pass
-    // has radix M/32: then the merged values go from registers straight into the pass
-    constexpr bool FIRST_IN_REGS = (SPEC != ZS_NONE) && (ct::radix_at(M, 0, false) == M / 32);
-    cplx xa[SPEC != ZS_NONE ? M / 32 : 1];
-    if constexpr (USE_A) {
-#pragma unroll
-        for (int i = 0; i < HB; ++i) a[i] = ld_stream(p + 32 * i + lane);
-    }
+
     if constexpr (SPEC != ZS_NONE) {
-        // Hermitian merge straight from global memory into the FFT buffer
+        // ---- Hermitian merge straight from global memory ----
+        // Z_k, k = lane + 32 t, is exactly what butterfly `lane` of the first inverse pass reads when that
+        // pass has radix M/32: then the merged values go from registers straight into the pass
+        constexpr bool FIRST_IN_REGS = (ct::radix_at(M, 0, false) == M / 32);
         const cplx* in = spec + (long long)line * (M + 1);
-        cplx xb[M / 32];
+        cplx xa[M / 32], xb[M / 32];
 #pragma unroll
         for (int t = 0; t < M / 32; ++t) {
             const int k = lane + 32 * t;
             xa[t] = ld_stream(in + k);
             xb[t] = ld_stream(in + (M - k));
-        }
-        if constexpr (USE_A) {
-#pragma unroll
-            for (int i = 0; i < HB; ++i) A[PL::at(32 * i + lane)] = a[i];
-#pragma unroll
-            for (int i = 0; i < HB; ++i) a[i] = ld_stream(p + 32 * (HB + i) + lane);
         }
 #pragma unroll
         for (int t = 0; t < M / 32; ++t) {
@@ -215,53 +210,12 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
             const cplx wd = cmul(w, d);
             xa[t] = mk(s.x - wd.y, s.y + wd.x);                   // Z_k = s + i w d
         }
-        if constexpr (!FIRST_IN_REGS) {
-#pragma unroll
-            for (int t = 0; t < M / 32; ++t) B[PosPad::at(lane + 32 * t)] = xa[t];
-        }
-        if constexpr (USE_A) {
-#pragma unroll
-            for (int i = 0; i < HB; ++i) A[PL::at(32 * (HB + i) + lane)] = a[i];
-        }
-    } else {
-#pragma unroll
-        for (int i = 0; i < HB; ++i) A[PL::at(32 * i + lane)] = a[i];
-#pragma unroll
-        for (int i = 0; i < HB; ++i) a[i] = ld_stream(p + 32 * (HB + i) + lane);
-#pragma unroll
-        for (int i = 0; i < HB; ++i) A[PL::at(32 * (HB + i) + lane)] = a[i];
-    }
-    __syncwarp();
-
-    if constexpr (SPEC != ZS_NONE) {
-        const int i = line / Z.ny, j = line - i * Z.ny;
-        const double vxy = __ldg(&Z.vx[i]) + __ldg(&Z.vy[j]);
-        const double s2 = Z.scal[SC_S2], s1 = Z.scal[SC_S1];
-        auto none = [](int) { return mk(0.0, 0.0); };
-        auto nonlin = [&](int m, cplx phi) {
-            if constexpr (SPEC == ZS_PHI) {
-                reinterpret_cast<double2*>(Z.phi_out + (long long)line * NZ)[m] = phi;
-            } else {
-                const double2 vz = __ldg(reinterpret_cast<const double2*>(Z.vz) + m);
-                const double vzz[2] = {vz.x, vz.y}, ph[2] = {phi.x, phi.y};
-#pragma unroll
-                for (int t = 0; t < 2; ++t) {
-                    const int pos = PL::at(2 * m + t);
-                    cplx a = A[pos];
-                    const double dens = s2 * cabs2(a);
-                    const double H = 0.5 * (vxy + vzz[t]) + Z.g * dens + Z.gdd * ph[t];
-                    if constexpr (SPEC == ZS_IMAG) {
-                        const double f = exp(-Z.dt * H) * s1;
-                        a = mk(f * a.x, f * a.y);
-                    } else {
-                        double sn, cs;
-                        sincos(Z.dt * H, &sn, &cs);
-                        a = mk(cs * a.x + sn * a.y, cs * a.y - sn * a.x);
-                    }
-                    A[pos] = a;
-                }
-            }
+        // the last pass leaves z_m = Phi_{2m} + i Phi_{2m+1} at B[m], unpadded: Phi as nz plain doubles
+        auto keep_phi = [&](int m, cplx phi) {
+            if constexpr (SPEC == ZS_PHI) reinterpret_cast<double2*>(Z.phi_out + (long long)line * NZ)[m] = phi;
+            else B[m] = phi;
         };
+        auto none = [](int) { return mk(0.0, 0.0); };
         if constexpr (FIRST_IN_REGS) {
             using P0 = CtPass<M, 0, true, false, 32>;
             static_assert(P0::NB == 1 && P0::R == M / 32 && P0::Ns == 1, "first pass must be one butterfly per lane");
@@ -270,52 +224,93 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
             for (int q = 0; q < P0::R; ++q) p0.v[0][q] = xa[q];
             p0.bfly(lane);
             if constexpr (P0::LAST) {
-                p0.scatter(lane, nonlin);
+                p0.scatter(lane, keep_phi);
             } else {
                 p0.scatter(lane, [&](int idx, cplx val) { B[PosPad::at(idx)] = val; });
                 __syncwarp();
-                ct_fft_range<M, true, false, 32, SyncWarp, PosPad, 1, L, false>(B, lane, true, Z.tw, none, nonlin);
+                ct_fft_range<M, true, false, 32, SyncWarp, PosPad, 1, L, false>(B, lane, true, Z.tw, none, keep_phi);
             }
         } else {
-            ct_fft_range<M, true, false, 32, SyncWarp, PosPad, 0, L, false>(B, lane, true, Z.tw, none, nonlin);
+#pragma unroll
+            for (int t = 0; t < M / 32; ++t) B[PosPad::at(lane + 32 * t)] = xa[t];
+            __syncwarp();
+            ct_fft_range<M, true, false, 32, SyncWarp, PosPad, 0, L, false>(B, lane, true, Z.tw, none, keep_phi);
         }
-        __syncwarp();
     }
+    __syncwarp();
+    if constexpr (!USE_A) return;
+    mbar_wait(&bars[warp], 0u);                          // the psi line has landed
 
+    // ---- psi_e after the nonlinear / potential exponential (or as it stands: ZS_NONE) ----
+    const double* Bd = reinterpret_cast<const double*>(B);
+    double vxy = 0.0, s2 = 1.0, s1 = 1.0;
+    if constexpr (SPEC != ZS_NONE) {
+        const int i = line / Z.ny, j = line - i * Z.ny;
+        vxy = __ldg(&Z.vx[i]) + __ldg(&Z.vy[j]);
+        s2 = Z.scal[SC_S2];
+        s1 = Z.scal[SC_S1];
+    }
+    auto upd = [&](int e) -> cplx {
+        cplx a = A[e];
+        if constexpr (SPEC == ZS_IMAG || SPEC == ZS_REAL) {
+            const double z = (double)(e - NZ / 2) * Z.dz;          // R#6
+            const double vz = Z.lam2 * z * z;
+            const double dens = s2 * cabs2(a);
+            const double H = 0.5 * (vxy + vz) + Z.g * dens + Z.gdd * Bd[e];
+            if constexpr (SPEC == ZS_IMAG) {
+                const double f = exp(-Z.dt * H) * s1;
+                a = mk(f * a.x, f * a.y);
+            } else {
+                double sn, cs;
+                sincos(Z.dt * H, &sn, &cs);
+                a = mk(cs * a.x + sn * a.y, cs * a.y - sn * a.x);
+            }
+        }
+        return a;
+    };
+
+    const int s = 1 + lane * LC;
+    const int cnt = min(LC, NZ - 1 - s);                  // unknowns of this lane's chunk (<= 0: idle lane)
     if constexpr (SWEEP) {
-        const int s = 1 + lane * LC;
-        const int cnt = min(LC, NZ - 1 - s);              // unknowns of this lane's chunk (<= 0: idle lane)
         const int Gn = T.G;
-        // table base of this lane: away from the left wall the elimination factors have converged to
-        // their fixed point, so the interior chunks share one set of entries (T.gU, decided on the host
-        // by a bitwise comparison) -- one broadcast address per load instead of 32 scattered ones
+        // table base of this lane (CONSTTAB = false): away from the left wall the elimination factors have
+        // converged, so the interior chunks share one set of entries (T.gU) -- one broadcast address
         const int sT = (lane >= T.gU && lane < Gn - 1) ? 1 + T.gU * LC : s;
         const bool l0 = lane == 0;
         auto t_inv = [&](int i) { if constexpr (CONSTTAB) return l0 ? P.inv0[i] : P.invU[i]; else return __ldg(&T.inv[sT + i]); };
         auto t_cc = [&](int i) { if constexpr (CONSTTAB) return l0 ? P.cc0[i] : P.ccU[i]; else return __ldg(&T.cc[sT + i]); };
         auto t_F = [&](int i) { if constexpr (CONSTTAB) return P.fU[i]; else return __ldg(&T.F[sT + i]); };
         auto t_Gm = [&](int i) { if constexpr (CONSTTAB) return l0 ? P.gm0[i] : P.gmU[i]; else return __ldg(&T.Gm[sT + i]); };
-        // ---- A: local forward elimination with zero inflow; end nodes read as zero (R#7, R#8) ----
+
+        // ---- A: nonlinear update on the fly + local forward elimination with zero inflow; the end nodes
+        //      of the line are read as zero (R#7, R#8).
+        // (branch-free: every lane evaluates its LC updates on clamped indices and masks the ones past its
+        // chunk or on an end node, so the exponentials of one lane interleave; the two halo values come
+        // from the neighbouring lanes by shuffles -- every lane left of an active lane owns a full chunk)
+        cplx pv[LC + 2];
+#pragma unroll
+        for (int i = 1; i <= LC; ++i) {
+            const int j = s - 1 + i;
+            const cplx v = upd(min(j, NZ - 1));
+            const bool in = (j <= NZ - 2);
+            pv[i] = mk(in ? v.x : 0.0, in ? v.y : 0.0);
+        }
+        {
+            const cplx up = shfl_c(pv[LC], (lane + 31) & 31), dn = shfl_c(pv[1], (lane + 1) & 31);
+            pv[0] = (lane == 0) ? mk(0.0, 0.0) : up;
+            pv[LC + 1] = (lane == 31) ? mk(0.0, 0.0) : dn;
+        }
         cplx ev[LC];
         cplx e = mk(0.0, 0.0);
-        {
-            cplx pm = (lane == 0 || cnt <= 0) ? mk(0.0, 0.0) : A[PL::at(s - 1)];
-            cplx p0 = (cnt > 0) ? A[PL::at(s)] : mk(0.0, 0.0);
 #pragma unroll
-            for (int i = 0; i < LC; ++i) {
-                ev[i] = mk(0.0, 0.0);
-                if (i < cnt) {
-                    const int jn = s + i + 1;
-                    const cplx pp = (jn < NZ - 1) ? A[PL::at(jn)] : mk(0.0, 0.0);
-                    // inv_j (d_j + r e_{j-1}) = inv_j d_j + (-c_j) e_{j-1}: one dependent fma per unknown
-                    cplx d = coef_mul(T.r, cadd(pm, pp));
-                    d = coef_fma(T.omr2, p0, d);
-                    e = coef_fma(coef_neg(t_cc(i)), e, coef_mul(t_inv(i), d));
-                    ev[i] = e;
-                    pm = p0;
-                    p0 = pp;
-                }
-            }
+        for (int i = 0; i < LC; ++i) {
+            // inv_j (d_j + r e_{j-1}) = inv_j d_j + (-c_j) e_{j-1}: one dependent fma per unknown
+            cplx d = coef_mul(T.r, cadd(pv[i], pv[i + 2]));
+            d = coef_fma(T.omr2, pv[i + 1], d);
+            const cplx en = coef_fma(coef_neg(t_cc(i)), e, coef_mul(t_inv(i), d));
+            const bool on = i < cnt;
+            e = mk(on ? en.x : e.x, on ? en.y : e.y);
+            ev[i] = e;
         }
         // ---- B: forward inflow by a look-back over the lanes to the left ----
         const CT Ag = (lane < Gn) ? __ldg(&T.Ach[lane]) : ct_zero(CT());
@@ -345,22 +340,29 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
             const CT Bh = shfl_ct(Bg, h & 31);
             if (h < Gn) xin = coef_fma(Bh, xin, Xh);
         }
-        __syncwarp();                                    // every lane has read its neighbours' values
+        __syncwarp();                                    // every lane has read its halo from the line buffer
         // ---- E: final values back into the line buffer; Dirichlet end nodes are exact zeros ----
 #pragma unroll
         for (int i = 0; i < LC; ++i)
-            if (i < cnt) A[PL::at(s + i)] = coef_fma(t_Gm(i), xin, ev[i]);
-        if (lane == 0) A[PL::at(0)] = mk(0.0, 0.0);
-        if (lane == 31) A[PL::at(NZ - 1)] = mk(0.0, 0.0);
-        __syncwarp();
+            if (i < cnt) A[s + i] = coef_fma(t_Gm(i), xin, ev[i]);
+        if (lane == 0) A[0] = mk(0.0, 0.0);
+        if (lane == 31) A[NZ - 1] = mk(0.0, 0.0);
+    } else {
+        // nonlinear update only (dgpe_nonlinear): every point of the line, end nodes included
+#pragma unroll
+        for (int i = 0; i < LC; ++i)
+            if (i < cnt) A[s + i] = upd(s + i);
+        if (lane == 0) A[0] = upd(0);
+        if (lane == 31) A[NZ - 1] = upd(NZ - 1);
     }
 
-    if constexpr (USE_A) {
-#pragma unroll
-        for (int i = 0; i < G::NPER; ++i) {
-            const int e = 32 * i + lane;
-            st_stream(p + e, A[PL::at(e)]);
-        }
+    // ---- the line goes back by one bulk store ----
+    fence_proxy_async();                                 // my writes -> visible to the async proxy
+    __syncwarp();
+    if (lane == 0) {
+        bulk_store(p, A, NZ * 16u);
+        tma_store_commit();
+        tma_store_wait_read<0>();                        // shared memory must outlive the copy
     }
 }
 
