@@ -36,8 +36,10 @@ def pair(gpu, oracle, shape, d, dt, trap, g, gdd, mode):
 
 # shapes span: one tile, ragged last tiles (line counts not multiples of 8), radix 3, several FFT passes,
 # nz = 2*odd, minimum size 4, non-cubic
+# (the last three: the 768- and 384-point kernels of BJ:configs[4] -- TMA-fed sweeps with 96 chunks per line,
+# four-pass FFTs with a radix-3 pass, the 384-point z-line kernels -- on thin boxes the oracle finishes fast)
 STAGE_SHAPES = [(4, 4, 4), (8, 8, 8), (6, 9, 12), (12, 18, 16), (27, 32, 6), (16, 24, 36), (64, 64, 64),
-                (48, 96, 128), (9, 4, 18)]
+                (48, 96, 128), (9, 4, 18), (768, 8, 64), (16, 768, 128), (8, 384, 384)]
 
 
 @pytest.mark.parametrize("shape", STAGE_SHAPES)
@@ -78,14 +80,16 @@ def test_stage_parity(gpu, oracle, shape, mode):
 @pytest.mark.parametrize("dt", [0.5, 5.0, 40.0])
 def test_sweeps_with_large_r_need_the_long_lookback(gpu, oracle, mode, dt):
     """r = dt/(4 d^2) up to 250: the chunk factors are O(1), so the inflow look-back spans many chunks."""
-    shape = (64, 48, 96)
-    G, O = pair(gpu, oracle, shape, (0.3, 0.25, 0.2), dt, (1.0, 1.0, 1.0), 0.0, 0.0, mode)
-    psi = inputs.random_state(shape, 5)
-    for axis in range(3):
-        t, a = dev(psi), psi.copy()
-        G.sweep(t, axis)
-        O.sweep(a, axis)
-        assert np.max(np.abs(t.cpu().numpy() - a)) <= 1e-12 * (1 + dt), axis
+    # (64, 48, 96): generic z kernel; (8, 384, 128): the TMA-fed y sweep and the warp-per-line z sweep, both
+    # reading the global tables because the elimination factors do not converge within a chunk
+    for shape in [(64, 48, 96), (8, 384, 128)]:
+        G, O = pair(gpu, oracle, shape, (0.3, 0.25, 0.2), dt, (1.0, 1.0, 1.0), 0.0, 0.0, mode)
+        psi = inputs.random_state(shape, 5)
+        for axis in range(3):
+            t, a = dev(psi), psi.copy()
+            G.sweep(t, axis)
+            O.sweep(a, axis)
+            assert np.max(np.abs(t.cpu().numpy() - a)) <= 1e-12 * (1 + dt), (shape, axis)
 
 
 def run_both(gpu, oracle, cfg, checkpoints, psi0=None):
@@ -218,6 +222,23 @@ def test_step_host_matches_device_path(gpu):
     hp = torch.from_numpy(psi0.copy()).pin_memory()
     assert G.step_host(hp, 3) == gpu.OK
     assert torch.equal(hp, t.cpu())                 # same kernels, deterministic reductions: bit-identical
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("env", ["DGPE_GENERIC=1", "DGPE_TMA=0", "DGPE_TMA=2", "DGPE_GRAPH=0", "DGPE_PREFETCH=0"])
+def test_kernel_variants_agree(gpu, monkeypatch, mode, env):
+    """The library carries two kernel sets (specialised and generic) and switches for
+    A/B runs; every variant must give the same step to rounding (different summation orders only)."""
+    shape = (64, 384, 128)
+    args = (*shape, 0.3, 0.25, 0.2, 0.004, 1.0, 0.7, 1.3, 5.0, 3.0, mode)
+    psi = inputs.random_state(shape, 21) * 0.05
+    ref = dev(psi)
+    gpu.Dgpe(*args).step(ref, 3)
+    name, val = env.split("=")
+    monkeypatch.setenv(name, val)
+    alt = dev(psi)
+    gpu.Dgpe(*args).step(alt, 3)
+    assert float((alt - ref).abs().max()) <= 1e-13
 
 
 def test_bitwise_repeatable(gpu):
