@@ -72,19 +72,47 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
     const double s2 = scal[SC_S2];
 
     const cplx* p = psi + (long long)line * NZ;
-    cplx a[G::NPER];
-#pragma unroll
-    for (int i = 0; i < G::NPER; ++i) a[i] = ld_stream(p + 32 * i + lane);
-#pragma unroll
-    for (int i = 0; i < G::NPER; ++i) {
-        const int e = 32 * i + lane, m = e >> 1;
-        Bd[2 * PosPad::at(m) + (e & 1)] = s2 * cabs2(a[i]);
-    }
-    __syncwarp();
-
     auto none = [](int) { return mk(0.0, 0.0); };
-    ct_fft_range<M, false, false, 32, SyncWarp, PosPad, 0, L, false>(
-        B, lane, true, tw, none, [&](int idx, cplx v) { B[PosPad::at(idx)] = v; });
+    auto keep = [&](int idx, cplx v) { B[PosPad::at(idx)] = v; };
+    // z_m, m = lane + 32 q, is exactly what butterfly `lane` of the first pass reads when that pass has
+    // radix M/32: then each lane loads its pairs (psi_{2m}, psi_{2m+1}) with one 256-bit load -- a warp
+    // reads 1 KB contiguous -- and the densities go from registers straight into the pass
+    constexpr bool FIRST_IN_REGS = (ct::radix_at(M, 0, false) == M / 32);
+    if constexpr (FIRST_IN_REGS) {
+        using P0 = CtPass<M, 0, false, false, 32>;
+        static_assert(P0::NB == 1 && P0::R == M / 32 && P0::Ns == 1, "first pass must be one butterfly per lane");
+        P0 p0;
+        double4 w[P0::R];
+#pragma unroll
+        for (int q = 0; q < P0::R; ++q) {
+            const double* src = reinterpret_cast<const double*>(p + 2 * (lane + 32 * q));
+            asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];\n"
+                         : "=d"(w[q].x), "=d"(w[q].y), "=d"(w[q].z), "=d"(w[q].w)
+                         : "l"(src));
+        }
+#pragma unroll
+        for (int q = 0; q < P0::R; ++q)
+            p0.v[0][q] = mk(s2 * (w[q].x * w[q].x + w[q].y * w[q].y), s2 * (w[q].z * w[q].z + w[q].w * w[q].w));
+        p0.bfly(lane);
+        if constexpr (P0::LAST) {
+            p0.scatter(lane, keep);
+        } else {
+            p0.scatter(lane, keep);
+            __syncwarp();
+            ct_fft_range<M, false, false, 32, SyncWarp, PosPad, 1, L, false>(B, lane, true, tw, none, keep);
+        }
+    } else {
+        cplx a[G::NPER];
+#pragma unroll
+        for (int i = 0; i < G::NPER; ++i) a[i] = ld_stream(p + 32 * i + lane);
+#pragma unroll
+        for (int i = 0; i < G::NPER; ++i) {
+            const int e = 32 * i + lane, m = e >> 1;
+            Bd[2 * PosPad::at(m) + (e & 1)] = s2 * cabs2(a[i]);
+        }
+        __syncwarp();
+        ct_fft_range<M, false, false, 32, SyncWarp, PosPad, 0, L, false>(B, lane, true, tw, none, keep);
+    }
     __syncwarp();
 
     cplx* out = spec + (long long)line * (M + 1);
