@@ -345,7 +345,7 @@ static int init_handle(dgpe_handle* h)
         // chunk length of the sweep recursions: 8 (or 16) unknowns per thread on the strided axes; on z
         // the warp-per-line kernel gives every lane ceil((nz-2)/32) unknowns
         int lc = (ns[a] <= 770 && !h->force_generic) ? 8 : 16;
-        if (a == 2 && h->zfast) lc = ((nz - 2 + 31) / 32) | 1;      // odd: conflict-free chunk walks (zline.cuh)
+        if (a == 2 && h->zfast) lc = ((nz - 2 + z_team(nz) - 1) / z_team(nz)) | 1;      // = ZGeom<nz>::LC, odd (zline.cuh)
         if (h->mode == DGPE_IMAG)
             rc = build_sweep<double>(h, &h->sw[a], ns[a], std::complex<double>(rr, 0.0), lc);
         else
@@ -501,7 +501,7 @@ static void fill_chunk_tabs(const AxisSweep& S, bool use, ChunkTabs<CT, LC>* P)
 template <int NZ>
 constexpr int z_main_minb(bool use_a, bool use_b)
 {
-    const int per_cta = 4 * ((use_a ? ZGeom<NZ>::A_ELEMS : 0) + (use_b ? ZGeom<NZ>::B_ELEMS : 0)) * 16 + 1024;
+    const int per_cta = 4 * ZGeom<NZ>::LPW * ((use_a ? ZGeom<NZ>::A_ELEMS : 0) + (use_b ? ZGeom<NZ>::B_ELEMS : 0)) * 16 + 1024;
     const int m = (227 * 1024) / per_cta;
     return m < 1 ? 1 : (m > 4 ? 4 : m);
 }
@@ -510,7 +510,8 @@ template <int NZ>
 static int launch_z_r2c_n(dgpe_handle* h, const cplx* psi)
 {
     constexpr int WARPS = 8;
-    const size_t smem = (size_t)WARPS * ZGeom<NZ>::B_ELEMS * sizeof(cplx);
+    constexpr int LINES = WARPS * ZGeom<NZ>::LPW;        // lines per CTA
+    const size_t smem = (size_t)LINES * ZGeom<NZ>::B_ELEMS * sizeof(cplx);
     auto kern = k_z_r2c<NZ, WARPS>;
     static bool ready = false;
     if (!ready) {
@@ -518,17 +519,17 @@ static int launch_z_r2c_n(dgpe_handle* h, const cplx* psi)
         ready = true;
     }
     const int nlines = h->nx * h->ny;
-    kern<<<(nlines + WARPS - 1) / WARPS, 32 * WARPS, smem, h->stream>>>(psi, h->spec, nlines, h->tw_zh, h->tw_split, h->scal);
+    kern<<<(nlines + LINES - 1) / LINES, 32 * WARPS, smem, h->stream>>>(psi, h->spec, nlines, h->tw_zh, h->tw_split, h->scal);
     return check_launch("k_z_r2c");
 }
 
 template <int NZ, typename CT, int SPEC, bool SWEEP, bool CONSTTAB>
 static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
 {
-    constexpr int WARPS = 4, LC = ZGeom<NZ>::LC;
+    constexpr int WARPS = 4, LC = ZGeom<NZ>::LC, LINES = WARPS * ZGeom<NZ>::LPW;
     constexpr bool USE_A = SPEC != ZS_PHI, USE_B = SPEC != ZS_NONE;
     constexpr int MINB = z_main_minb<NZ>(USE_A, USE_B);
-    const size_t smem = (size_t)WARPS * ((USE_A ? ZGeom<NZ>::A_ELEMS : 0) + (USE_B ? ZGeom<NZ>::B_ELEMS : 0)) * sizeof(cplx);
+    const size_t smem = (size_t)LINES * ((USE_A ? ZGeom<NZ>::A_ELEMS : 0) + (USE_B ? ZGeom<NZ>::B_ELEMS : 0)) * sizeof(cplx);
     auto kern = k_z_main<NZ, CT, SPEC, SWEEP, CONSTTAB, WARPS, MINB>;
     static bool ready = false;
     if (!ready) {
@@ -542,7 +543,7 @@ static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
     T.inv = (const CT*)S.inv; T.cc = (const CT*)S.cc; T.F = (const CT*)S.F; T.Gm = (const CT*)S.Gm;
     T.Ach = (const CT*)S.Ach; T.Bch = (const CT*)S.Bch;
     T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb; T.gU = S.gU;
-    if (SWEEP && (S.Lc != LC || S.G > 32)) return fail(DGPE_ERR_CUDA, "z sweep tables do not match the z-line kernel");
+    if (SWEEP && (S.Lc != LC || S.G > ZGeom<NZ>::T)) return fail(DGPE_ERR_CUDA, "z sweep tables do not match the z-line kernel");
     ChunkTabs<CT, LC> P;
     fill_chunk_tabs<CT, LC>(S, SWEEP && CONSTTAB, &P);
     ZMainArgs Z;
@@ -554,9 +555,9 @@ static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
     {
         static int ctas_per_sm = 0;
         if (!ctas_per_sm) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, 32 * WARPS, smem));
-        Z.pf_lines = (h->prefetch & PF_Z) ? h->pf_mult * ctas_per_sm * h->num_sms * WARPS : 0;
+        Z.pf_lines = (h->prefetch & PF_Z) ? h->pf_mult * ctas_per_sm * h->num_sms * LINES : 0;
     }
-    kern<<<(Z.nlines + WARPS - 1) / WARPS, 32 * WARPS, smem, h->stream>>>(psi, h->spec, Z, T, P);
+    kern<<<(Z.nlines + LINES - 1) / LINES, 32 * WARPS, smem, h->stream>>>(psi, h->spec, Z, T, P);
     return check_launch("k_z_main");
 }
 

@@ -29,11 +29,23 @@
 
 namespace dgpe {
 
+// Lanes per line.  The long lines take a whole warp; for nz/2 = 32 .. 256 (a power of two) a TEAM of
+// T = nz/16 lanes owns a line -- then the first FFT pass is one radix-8 butterfly per lane, every lane
+// holds 16 psi elements and 17 sweep unknowns exactly as at nz = 512, and a warp works on 32/T lines at
+// once with no idle lanes (BJ:configs[0..2]: nz = 64, 128, 256).
+__host__ __device__ constexpr int z_team(int nz)
+{
+    const int m = nz / 2;
+    return (m == 32 || m == 64 || m == 128 || m == 256) ? m / 8 : 32;
+}
+
 template <int NZ>
 struct ZGeom {
     static constexpr int M = NZ / 2;
-    static constexpr int NPER = NZ / 32;                       // psi elements per lane (coalesced walks)
-    static constexpr int LC = ((NZ - 2 + 31) / 32) | 1;        // sweep chunk per lane, odd
+    static constexpr int T = z_team(NZ);                       // lanes per line
+    static constexpr int LPW = 32 / T;                         // lines per warp
+    static constexpr int NPER = NZ / T;                        // psi elements per lane (coalesced walks)
+    static constexpr int LC = ((NZ - 2 + T - 1) / T) | 1;      // sweep chunk per lane, odd
     static constexpr int A_ELEMS = NZ;
     static constexpr int B_ELEMS = (M + (M >> 3) + 7) / 8 * 8;
     static_assert(NZ % 64 == 0, "z-line kernels need nz to be a multiple of 64");
@@ -43,10 +55,15 @@ struct PosPad {
     static __device__ __forceinline__ int at(int idx) { return idx + (idx >> 3); }
 };
 
-__device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
-__device__ __forceinline__ cplx shfl_c(cplx v, int src) { return mk(shfl_d(v.x, src), shfl_d(v.y, src)); }
-__device__ __forceinline__ double shfl_ct(double v, int src) { return shfl_d(v, src); }
-__device__ __forceinline__ cplx shfl_ct(cplx v, int src) { return shfl_c(v, src); }
+// shuffles inside a team of W lanes (src = lane index within the team)
+template <int W>
+__device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src, W); }
+template <int W>
+__device__ __forceinline__ cplx shfl_c(cplx v, int src) { return mk(shfl_d<W>(v.x, src), shfl_d<W>(v.y, src)); }
+template <int W>
+__device__ __forceinline__ double shfl_ct(double v, int src) { return shfl_d<W>(v, src); }
+template <int W>
+__device__ __forceinline__ cplx shfl_ct(cplx v, int src) { return shfl_c<W>(v, src); }
 __device__ __forceinline__ double ct_zero(double) { return 0.0; }
 __device__ __forceinline__ cplx ct_zero(cplx) { return mk(0.0, 0.0); }
 
@@ -54,7 +71,7 @@ __device__ __forceinline__ cplx ct_zero(cplx) { return mk(0.0, 0.0); }
 // K1: density + real-to-complex transform along z.  With M = nz/2 the real line is packed as
 // z_m = n_{2m} + i n_{2m+1}; Z = DFT_M(z); X_k = (Z_k + conj Z_{M-k})/2 - (i/2) e^{-2 pi i k/nz}
 // (Z_k - conj Z_{M-k}), k = 0..M, Z_M := Z_0.   tws[k] = exp(-2 pi i k/nz).
-// grid = ceil(nlines / WARPS); block = 32*WARPS; dynamic shared memory = WARPS * B_ELEMS * 16 bytes.
+// grid = ceil(nlines / (WARPS LPW)); block = 32*WARPS; dynamic shared memory = WARPS LPW B_ELEMS 16 bytes.
 // ------------------------------------------------------------------------------------------------
 template <int NZ, int WARPS>
 __global__ void __launch_bounds__(32 * WARPS)
@@ -62,30 +79,32 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
         const cplx* __restrict__ tws, const double* __restrict__ scal)
 {
     using G = ZGeom<NZ>;
-    constexpr int M = G::M, L = ct::npass(M);
+    constexpr int M = G::M, L = ct::npass(M), TL = G::T, LPW = G::LPW;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int line = blockIdx.x * WARPS + warp;
-    if (line >= nlines) return;                         // warps are independent: no block barrier below
-    cplx* B = reinterpret_cast<cplx*>(smem_raw) + (size_t)warp * G::B_ELEMS;
+    const int warp = threadIdx.x >> 5, team = (threadIdx.x & 31) / TL, lane = threadIdx.x & (TL - 1);   // lane within the team
+    const int line0 = (blockIdx.x * WARPS + warp) * LPW;
+    if (line0 >= nlines) return;                        // warps are independent: no block barrier below
+    const bool valid = line0 + team < nlines;           // a team past the end works on the last line, stores nothing
+    const int line = valid ? line0 + team : nlines - 1;
+    cplx* B = reinterpret_cast<cplx*>(smem_raw) + (size_t)(warp * LPW + team) * G::B_ELEMS;
     double* Bd = reinterpret_cast<double*>(B);
     const double s2 = scal[SC_S2];
 
     const cplx* p = psi + (long long)line * NZ;
     auto none = [](int) { return mk(0.0, 0.0); };
     auto keep = [&](int idx, cplx v) { B[PosPad::at(idx)] = v; };
-    // z_m, m = lane + 32 q, is exactly what butterfly `lane` of the first pass reads when that pass has
-    // radix M/32: then each lane loads its pairs (psi_{2m}, psi_{2m+1}) with one 256-bit load -- a warp
+    // z_m, m = lane + TL q, is exactly what butterfly `lane` of the first pass reads when that pass has
+    // radix M/TL: then each lane loads its pairs (psi_{2m}, psi_{2m+1}) with one 256-bit load -- a warp
     // reads 1 KB contiguous -- and the densities go from registers straight into the pass
-    constexpr bool FIRST_IN_REGS = (ct::radix_at(M, 0, false) == M / 32);
+    constexpr bool FIRST_IN_REGS = (ct::radix_at(M, 0, false) == M / TL);
     if constexpr (FIRST_IN_REGS) {
-        using P0 = CtPass<M, 0, false, false, 32>;
-        static_assert(P0::NB == 1 && P0::R == M / 32 && P0::Ns == 1, "first pass must be one butterfly per lane");
+        using P0 = CtPass<M, 0, false, false, TL>;
+        static_assert(P0::NB == 1 && P0::R == M / TL && P0::Ns == 1, "first pass must be one butterfly per lane");
         P0 p0;
         double4 w[P0::R];
 #pragma unroll
         for (int q = 0; q < P0::R; ++q) {
-            const double* src = reinterpret_cast<const double*>(p + 2 * (lane + 32 * q));
+            const double* src = reinterpret_cast<const double*>(p + 2 * (lane + TL * q));
             asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];\n"
                          : "=d"(w[q].x), "=d"(w[q].y), "=d"(w[q].z), "=d"(w[q].w)
                          : "l"(src));
@@ -99,19 +118,19 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
         } else {
             p0.scatter(lane, keep);
             __syncwarp();
-            ct_fft_range<M, false, false, 32, SyncWarp, PosPad, 1, L, false>(B, lane, true, tw, none, keep);
+            ct_fft_range<M, false, false, TL, SyncWarp, PosPad, 1, L, false>(B, lane, true, tw, none, keep);
         }
     } else {
         cplx a[G::NPER];
 #pragma unroll
-        for (int i = 0; i < G::NPER; ++i) a[i] = ld_stream(p + 32 * i + lane);
+        for (int i = 0; i < G::NPER; ++i) a[i] = ld_stream(p + TL * i + lane);
 #pragma unroll
         for (int i = 0; i < G::NPER; ++i) {
-            const int e = 32 * i + lane, m = e >> 1;
+            const int e = TL * i + lane, m = e >> 1;
             Bd[2 * PosPad::at(m) + (e & 1)] = s2 * cabs2(a[i]);
         }
         __syncwarp();
-        ct_fft_range<M, false, false, 32, SyncWarp, PosPad, 0, L, false>(B, lane, true, tw, none, keep);
+        ct_fft_range<M, false, false, TL, SyncWarp, PosPad, 0, L, false>(B, lane, true, tw, none, keep);
     }
     __syncwarp();
 
@@ -123,10 +142,10 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
         const cplx w = __ldg(&tws[k]);
         const cplx s = cadd(zk, zm), d = csub(zk, zm);
         const cplx wd = cmul(w, d);
-        st_stream(out + k, mk(0.5 * (s.x + wd.y), 0.5 * (s.y - wd.x)));     // s/2 - (i/2) w d
+        if (valid) st_stream(out + k, mk(0.5 * (s.x + wd.y), 0.5 * (s.y - wd.x)));     // s/2 - (i/2) w d
     };
 #pragma unroll
-    for (int t = 0; t < M / 32; ++t) split(lane + 32 * t);
+    for (int t = 0; t < M / TL; ++t) split(lane + TL * t);
     if (lane == 0) split(M);
 }
 
@@ -145,7 +164,7 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
 // Phi_{2m+1} = Im z_m.   H = V + g n + gdd Phi, n = s2 |psi|^2, V = (vx[i] + vy[j] + vz[k])/2.
 // Sweep: as sweep.cuh; lane l owns the unknowns 1 + l LC .. and keeps them in registers through the
 // forward elimination, the back substitution and the fix-up; the chunk outflows travel by shuffles.
-// grid = ceil(nlines / WARPS); block = 32*WARPS; dynamic smem = WARPS*(A_ELEMS + B_ELEMS)*16 bytes.
+// grid = ceil(nlines / (WARPS LPW)); block = 32*WARPS; dynamic smem = WARPS LPW (A_ELEMS + B_ELEMS) 16 bytes.
 // ------------------------------------------------------------------------------------------------
 enum { ZS_NONE = 0, ZS_IMAG = 1, ZS_REAL = 2, ZS_PHI = 3 };
 
@@ -183,55 +202,58 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
          const __grid_constant__ ChunkTabs<CT, ZGeom<NZ>::LC> P)
 {
     using G = ZGeom<NZ>;
-    constexpr int M = G::M, L = ct::npass(M), LC = G::LC;
+    constexpr int M = G::M, L = ct::npass(M), LC = G::LC, TL = G::T, LPW = G::LPW;
     constexpr bool USE_A = (SPEC != ZS_PHI);
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ __align__(8) unsigned long long bars[WARPS];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int line = blockIdx.x * WARPS + warp;
-    if (line >= Z.nlines) return;                       // warps are independent: no block barrier below
-    constexpr int PER_WARP = (USE_A ? G::A_ELEMS : 0) + (SPEC != ZS_NONE ? G::B_ELEMS : 0);
-    cplx* A = reinterpret_cast<cplx*>(smem_raw) + (size_t)warp * PER_WARP;
+    __shared__ __align__(8) unsigned long long bars[WARPS * LPW];
+    const int warp = threadIdx.x >> 5, team = (threadIdx.x & 31) / TL, lane = threadIdx.x & (TL - 1);   // lane within the team
+    const int line0 = (blockIdx.x * WARPS + warp) * LPW;
+    if (line0 >= Z.nlines) return;                      // warps are independent: no block barrier below
+    const bool valid = line0 + team < Z.nlines;         // a team past the end works on the last line, stores nothing
+    const int line = valid ? line0 + team : Z.nlines - 1;
+    const int slot = warp * LPW + team;
+    constexpr int PER_LINE = (USE_A ? G::A_ELEMS : 0) + (SPEC != ZS_NONE ? G::B_ELEMS : 0);
+    cplx* A = reinterpret_cast<cplx*>(smem_raw) + (size_t)slot * PER_LINE;
     cplx* B = A + (USE_A ? G::A_ELEMS : 0);
     cplx* p = psi + (long long)line * NZ;
 
     // ---- the psi line: one bulk copy, in flight while the spectrum is loaded, merged and transformed ----
     if constexpr (USE_A) {
         if (lane == 0) {
-            mbar_init(&bars[warp], 1);
+            mbar_init(&bars[slot], 1);
             mbar_fence_init();
-            mbar_expect_tx(&bars[warp], NZ * 16u);
-            bulk_load(A, p, NZ * 16u, &bars[warp]);
+            mbar_expect_tx(&bars[slot], NZ * 16u);
+            bulk_load(A, p, NZ * 16u, &bars[slot]);
         }
     }
     // ---- L2 prefetch for the warp that will run one residency later ----
     if (Z.pf_lines > 0 && line + Z.pf_lines < Z.nlines) {
         const char* pp = reinterpret_cast<const char*>(psi + (long long)(line + Z.pf_lines) * NZ);
         if constexpr (USE_A) {
-            for (int o = 128 * lane; o < NZ * 16; o += 128 * 32) prefetch_l2(pp + o);
+            for (int o = 128 * lane; o < NZ * 16; o += 128 * TL) prefetch_l2(pp + o);
         }
         if constexpr (SPEC != ZS_NONE) {
             const char* ps = reinterpret_cast<const char*>(spec + (long long)(line + Z.pf_lines) * (M + 1));
-            for (int o = 128 * lane; o < (M + 1) * 16; o += 128 * 32) prefetch_l2(ps + o);
+            for (int o = 128 * lane; o < (M + 1) * 16; o += 128 * TL) prefetch_l2(ps + o);
         }
     }
 
     if constexpr (SPEC != ZS_NONE) {
         // ---- Hermitian merge straight from global memory ----
-        // Z_k, k = lane + 32 t, is exactly what butterfly `lane` of the first inverse pass reads when that
-        // pass has radix M/32: then the merged values go from registers straight into the pass
-        constexpr bool FIRST_IN_REGS = (ct::radix_at(M, 0, false) == M / 32);
+        // Z_k, k = lane + TL t, is exactly what butterfly `lane` of the first inverse pass reads when that
+        // pass has radix M/TL: then the merged values go from registers straight into the pass
+        constexpr bool FIRST_IN_REGS = (ct::radix_at(M, 0, false) == M / TL);
         const cplx* in = spec + (long long)line * (M + 1);
-        cplx xa[M / 32], xb[M / 32];
+        cplx xa[M / TL], xb[M / TL];
 #pragma unroll
-        for (int t = 0; t < M / 32; ++t) {
-            const int k = lane + 32 * t;
+        for (int t = 0; t < M / TL; ++t) {
+            const int k = lane + TL * t;
             xa[t] = ld_stream(in + k);
             xb[t] = ld_stream(in + (M - k));
         }
 #pragma unroll
-        for (int t = 0; t < M / 32; ++t) {
-            const int k = lane + 32 * t;
+        for (int t = 0; t < M / TL; ++t) {
+            const int k = lane + TL * t;
             const cplx w = cconj(__ldg(&Z.tws[k]));               // e^{+2 pi i k/nz}
             const cplx cb = cconj(xb[t]);
             const cplx s = cadd(xa[t], cb), d = csub(xa[t], cb);
@@ -240,13 +262,13 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         }
         // the last pass leaves z_m = Phi_{2m} + i Phi_{2m+1} at B[m], unpadded: Phi as nz plain doubles
         auto keep_phi = [&](int m, cplx phi) {
-            if constexpr (SPEC == ZS_PHI) reinterpret_cast<double2*>(Z.phi_out + (long long)line * NZ)[m] = phi;
+            if constexpr (SPEC == ZS_PHI) { if (valid) reinterpret_cast<double2*>(Z.phi_out + (long long)line * NZ)[m] = phi; }
             else B[m] = phi;
         };
         auto none = [](int) { return mk(0.0, 0.0); };
         if constexpr (FIRST_IN_REGS) {
-            using P0 = CtPass<M, 0, true, false, 32>;
-            static_assert(P0::NB == 1 && P0::R == M / 32 && P0::Ns == 1, "first pass must be one butterfly per lane");
+            using P0 = CtPass<M, 0, true, false, TL>;
+            static_assert(P0::NB == 1 && P0::R == M / TL && P0::Ns == 1, "first pass must be one butterfly per lane");
             P0 p0;
 #pragma unroll
             for (int q = 0; q < P0::R; ++q) p0.v[0][q] = xa[q];
@@ -256,18 +278,18 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
             } else {
                 p0.scatter(lane, [&](int idx, cplx val) { B[PosPad::at(idx)] = val; });
                 __syncwarp();
-                ct_fft_range<M, true, false, 32, SyncWarp, PosPad, 1, L, false>(B, lane, true, Z.tw, none, keep_phi);
+                ct_fft_range<M, true, false, TL, SyncWarp, PosPad, 1, L, false>(B, lane, true, Z.tw, none, keep_phi);
             }
         } else {
 #pragma unroll
-            for (int t = 0; t < M / 32; ++t) B[PosPad::at(lane + 32 * t)] = xa[t];
+            for (int t = 0; t < M / TL; ++t) B[PosPad::at(lane + TL * t)] = xa[t];
             __syncwarp();
-            ct_fft_range<M, true, false, 32, SyncWarp, PosPad, 0, L, false>(B, lane, true, Z.tw, none, keep_phi);
+            ct_fft_range<M, true, false, TL, SyncWarp, PosPad, 0, L, false>(B, lane, true, Z.tw, none, keep_phi);
         }
     }
     __syncwarp();
     if constexpr (!USE_A) return;
-    mbar_wait(&bars[warp], 0u);                          // the psi line has landed
+    mbar_wait(&bars[slot], 0u);                          // the psi line has landed
 
     // ---- psi_e after the nonlinear / potential exponential (or as it stands: ZS_NONE) ----
     const double* Bd = reinterpret_cast<const double*>(B);
@@ -324,9 +346,9 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
             pv[i] = mk(in ? v.x : 0.0, in ? v.y : 0.0);
         }
         {
-            const cplx up = shfl_c(pv[LC], (lane + 31) & 31), dn = shfl_c(pv[1], (lane + 1) & 31);
+            const cplx up = shfl_c<TL>(pv[LC], (lane + TL - 1) & (TL - 1)), dn = shfl_c<TL>(pv[1], (lane + 1) & (TL - 1));
             pv[0] = (lane == 0) ? mk(0.0, 0.0) : up;
-            pv[LC + 1] = (lane == 31) ? mk(0.0, 0.0) : dn;
+            pv[LC + 1] = (lane == TL - 1) ? mk(0.0, 0.0) : dn;
         }
         cplx ev[LC];
         cplx e = mk(0.0, 0.0);
@@ -346,8 +368,8 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         cplx ein = mk(0.0, 0.0);
         for (int d = T.Kf; d >= 1; --d) {
             const int h = lane - d;
-            const cplx Eh = shfl_c(e, h & 31);
-            const CT Ah = shfl_ct(Ag, h & 31);
+            const cplx Eh = shfl_c<TL>(e, h & (TL - 1));
+            const CT Ah = shfl_ct<TL>(Ag, h & (TL - 1));
             if (h >= 0) ein = coef_fma(Ah, ein, Eh);
         }
         // ---- C: local back substitution with zero inflow ----
@@ -364,8 +386,8 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         cplx xin = mk(0.0, 0.0);
         for (int d = T.Kb; d >= 1; --d) {
             const int h = lane + d;
-            const cplx Xh = shfl_c(x, h & 31);
-            const CT Bh = shfl_ct(Bg, h & 31);
+            const cplx Xh = shfl_c<TL>(x, h & (TL - 1));
+            const CT Bh = shfl_ct<TL>(Bg, h & (TL - 1));
             if (h < Gn) xin = coef_fma(Bh, xin, Xh);
         }
         __syncwarp();                                    // every lane has read its halo from the line buffer
@@ -374,20 +396,20 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         for (int i = 0; i < LC; ++i)
             if (i < cnt) A[s + i] = coef_fma(t_Gm(i), xin, ev[i]);
         if (lane == 0) A[0] = mk(0.0, 0.0);
-        if (lane == 31) A[NZ - 1] = mk(0.0, 0.0);
+        if (lane == TL - 1) A[NZ - 1] = mk(0.0, 0.0);
     } else {
         // nonlinear update only (dgpe_nonlinear): every point of the line, end nodes included
 #pragma unroll
         for (int i = 0; i < LC; ++i)
             if (i < cnt) A[s + i] = upd(s + i);
         if (lane == 0) A[0] = upd(0);
-        if (lane == 31) A[NZ - 1] = upd(NZ - 1);
+        if (lane == TL - 1) A[NZ - 1] = upd(NZ - 1);
     }
 
     // ---- the line goes back by one bulk store ----
     fence_proxy_async();                                 // my writes -> visible to the async proxy
     __syncwarp();
-    if (lane == 0) {
+    if (lane == 0 && valid) {
         bulk_store(p, A, NZ * 16u);
         tma_store_commit();
         tma_store_wait_read<0>();                        // shared memory must outlive the copy
