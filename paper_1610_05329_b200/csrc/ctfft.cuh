@@ -7,7 +7,7 @@
 //     v_q = in[j + q N/R] w_N^{q k N/(Ns R)},    out[(j div Ns) Ns R + k + s Ns] = sum_q v_q w_R^{q s}.
 // Here N and the radix sequence are template constants, so every index folds at compile time and a
 // thread keeps its butterflies in registers between the read side and the write side of a pass.
-// The radix sequence is 8.., 4, 2, 3.. (REV = false) or its reverse (REV = true).  With the reversed
+// The radix sequence is 8.., 4, 2, 3.., 5.., 7.. (REV = false) or its reverse (REV = true).  With the reversed
 // sequence the first pass of a transform reads exactly the elements the last pass of a forward-order
 // transform produced in the same thread, so a forward and an inverse transform chain in registers
 // (K3: FFT_x, multiply by Udd~(k), IFFT_x -- BJ:north_star).
@@ -17,7 +17,10 @@
 namespace dgpe {
 namespace ct {
 
-__host__ __device__ constexpr int pick(int m) { return (m % 8 == 0) ? 8 : (m % 4 == 0) ? 4 : (m % 2 == 0) ? 2 : 3; }
+__host__ __device__ constexpr int pick(int m)
+{
+    return (m % 8 == 0) ? 8 : (m % 4 == 0) ? 4 : (m % 2 == 0) ? 2 : (m % 3 == 0) ? 3 : (m % 5 == 0) ? 5 : 7;
+}
 __host__ __device__ constexpr int npass(int n)
 {
     int c = 0;
@@ -47,6 +50,8 @@ __host__ __device__ constexpr bool smooth(int n)
     if (n < 1) return false;
     while (n % 2 == 0) n /= 2;
     while (n % 3 == 0) n /= 3;
+    while (n % 5 == 0) n /= 5;
+    while (n % 7 == 0) n /= 7;
     return n == 1;
 }
 
@@ -101,12 +106,10 @@ struct CtPass {
 #pragma unroll
                 for (int q = 0; q < R; ++q) v[u][q] = f(j + q * NBUT);
                 if constexpr (Ns > 1) {
-                    if (R >= 4) w[u][3] = cmul(w[u][1], w[u][2]);
-                    if (R == 8) {
-                        w[u][5] = cmul(w[u][1], w[u][4]);
-                        w[u][6] = cmul(w[u][2], w[u][4]);
-                        w[u][7] = cmul(w[u][3], w[u][4]);
-                    }
+                    if constexpr (R >= 4) w[u][3] = cmul(w[u][1], w[u][2]);
+                    if constexpr (R >= 6) w[u][5] = cmul(w[u][1], w[u][4]);
+                    if constexpr (R >= 7) w[u][6] = cmul(w[u][2], w[u][4]);
+                    if constexpr (R >= 8) w[u][7] = cmul(w[u][3], w[u][4]);
 #pragma unroll
                     for (int q = 1; q < R; ++q) v[u][q] = cmul(v[u][q], w[u][q]);
                 }

@@ -126,22 +126,23 @@ static int upload(dgpe_handle* h, const std::vector<T>& v, T** out)
     return DGPE_OK;
 }
 
-static bool smooth23(int n)
+// FFT-friendly sizes built so far: 2^a 3^b 5^c 7^d (P:L130 also lists 11 and 13)
+static bool smooth2357(int n)
 {
     if (n < 1) return false;
-    while (n % 2 == 0) n /= 2;
-    while (n % 3 == 0) n /= 3;
+    for (int f : {2, 3, 5, 7})
+        while (n % f == 0) n /= f;
     return n == 1;
 }
 
-// radices 8, 4, 2 first, 3 last; butterfly slots per column = n / largest radix
+// radices 8, 4, 2 first, then 3, 5, 7; butterfly slots per column = n / largest radix
 static int make_plan(dgpe_handle* h, int n, FftPlan* P, cplx** tw_dev)
 {
     std::memset(P, 0, sizeof(*P));
     P->n = n;
     int m = n, np = 0, rmax = 1;
-    const int order[4] = {8, 4, 2, 3};
-    for (int oi = 0; oi < 4; ++oi) {
+    const int order[6] = {8, 4, 2, 3, 5, 7};
+    for (int oi = 0; oi < 6; ++oi) {
         const int R = order[oi];
         while (m % R == 0 && m > 1) {
             if (np >= MAX_PASSES) return fail(DGPE_ERR_UNSUPPORTED, "FFT length %d needs too many passes", n);
@@ -150,7 +151,7 @@ static int make_plan(dgpe_handle* h, int n, FftPlan* P, cplx** tw_dev)
             if (R > rmax) rmax = R;
         }
     }
-    if (m != 1) return fail(DGPE_ERR_ARG, "FFT length %d is not of the form 2^a 3^b", n);
+    if (m != 1) return fail(DGPE_ERR_ARG, "FFT length %d is not of the form 2^a 3^b 5^c 7^d", n);
     if (np == 0) {           // n == 1: one radix-1 "pass" does not exist; callers never ask for it
         return fail(DGPE_ERR_ARG, "FFT length %d too small", n);
     }
@@ -405,7 +406,7 @@ extern "C" dgpe_handle* dgpe_create(int nx, int ny, int nz, double dx, double dy
     const int ns[3] = {nx, ny, nz};
     for (int a = 0; a < 3; ++a) {
         if (ns[a] < 4) { fail(DGPE_ERR_ARG, "grid size %d < 4", ns[a]); return nullptr; }
-        if (!smooth23(ns[a])) { fail(DGPE_ERR_ARG, "grid size %d is not of the form 2^a 3^b", ns[a]); return nullptr; }
+        if (!smooth2357(ns[a])) { fail(DGPE_ERR_ARG, "grid size %d is not of the form 2^a 3^b 5^c 7^d", ns[a]); return nullptr; }
         if (ns[a] > DGPE_MAX_N) { fail(DGPE_ERR_UNSUPPORTED, "grid size %d > %d", ns[a], DGPE_MAX_N); return nullptr; }
     }
     if (nz % 2) { fail(DGPE_ERR_ARG, "nz = %d must be even", nz); return nullptr; }
@@ -470,7 +471,7 @@ static int check_launch(const char* what)
 // ------------------------------------------------------------------------------------------------
 // warp-per-line z kernels (zline.cuh): specialised line lengths
 // ------------------------------------------------------------------------------------------------
-#define DGPE_Z_SIZES(X) X(64) X(128) X(192) X(256) X(384) X(512) X(768)
+#define DGPE_Z_SIZES(X) X(64) X(128) X(160) X(192) X(240) X(250) X(256) X(320) X(384) X(480) X(500) X(512) X(640) X(768)
 
 static bool z_specialised(int nz)
 {
@@ -649,11 +650,18 @@ static int launch_fft_xy(dgpe_handle* h, int n, const LineMap& map, int nbatch, 
         case 64: return launch_fft_xy_n<64, KIND>(h, map, nbatch, tw);
         case 96: return launch_fft_xy_n<96, KIND>(h, map, nbatch, tw);
         case 128: return launch_fft_xy_n<128, KIND>(h, map, nbatch, tw);
+        case 160: return launch_fft_xy_n<160, KIND>(h, map, nbatch, tw);
         case 192: return launch_fft_xy_n<192, KIND>(h, map, nbatch, tw);
+        case 240: return launch_fft_xy_n<240, KIND>(h, map, nbatch, tw);
         case 256: return launch_fft_xy_n<256, KIND>(h, map, nbatch, tw);
+        case 320: return launch_fft_xy_n<320, KIND>(h, map, nbatch, tw);
         case 384: return launch_fft_xy_n<384, KIND>(h, map, nbatch, tw);
+        case 480: return launch_fft_xy_n<480, KIND>(h, map, nbatch, tw);
+        case 500: return launch_fft_xy_n<500, KIND>(h, map, nbatch, tw);
         case 512: return launch_fft_xy_n<512, KIND>(h, map, nbatch, tw);
+        case 640: return launch_fft_xy_n<640, KIND>(h, map, nbatch, tw);
         case 768: return launch_fft_xy_n<768, KIND>(h, map, nbatch, tw);
+        case 960: return launch_fft_xy_n<960, KIND>(h, map, nbatch, tw);
         case 1024: return launch_fft_xy_n<1024, KIND>(h, map, nbatch, tw);
         default: *handled = false; return DGPE_OK;
     }

@@ -1,5 +1,5 @@
-// fft.cuh -- mixed-radix (2, 3, 4, 8) Stockham autosort FFT passes over a shared-memory tile of
-// TILE_COLS lines (FFT-friendly sizes 2^a 3^b ...; BJ:north_star "mixed-radix (2^a 3^b)
+// fft.cuh -- mixed-radix (2, 3, 4, 5, 7, 8) Stockham autosort FFT passes over a shared-memory tile of
+// TILE_COLS lines (FFT-friendly sizes 2^a 3^b 5^c 7^d ...; BJ:north_star "mixed-radix (2^a 3^b)
 // shared-memory Stockham FFT passes per axis").
 //
 // Pass p of an n-point transform with radix R and Ns = product of the radices of the passes before it:
@@ -49,6 +49,71 @@ struct Butterfly<3, INV> {
         v[0] = cadd(v[0], t1);
         v[1] = cadd(m1, m2);
         v[2] = csub(m1, m2);
+    }
+};
+
+// Odd prime radix R = 2h+1 (5, 7; P:L130 lists 2^a 3^b 5^c 7^d ... as the FFT-friendly sizes): with
+// a_k = v_k + v_{R-k}, b_k = v_k - v_{R-k}  (k = 1..h)
+//   out_s, out_{R-s} = (v_0 + sum_k cos(2 pi s k/R) a_k)  -/+  i sum_k sin(2 pi s k/R) b_k   (forward; signs swap for the inverse)
+template <int R, bool INV>
+struct OddPrimeButterfly {
+    static __device__ __forceinline__ void run(cplx (&v)[R], const double (&C)[R], const double (&S)[R])
+    {
+        constexpr int H = (R - 1) / 2;
+        cplx a[H], b[H];
+#pragma unroll
+        for (int k = 1; k <= H; ++k) {
+            a[k - 1] = cadd(v[k], v[R - k]);
+            b[k - 1] = csub(v[k], v[R - k]);
+        }
+        cplx sum = v[0];
+#pragma unroll
+        for (int k = 0; k < H; ++k) sum = cadd(sum, a[k]);
+        cplx out[R];
+        out[0] = sum;
+#pragma unroll
+        for (int s = 1; s <= H; ++s) {
+            cplx re = v[0], im = mk(0.0, 0.0);
+#pragma unroll
+            for (int k = 1; k <= H; ++k) {
+                const int m = (s * k) % R;
+                re = mk(fma(C[m], a[k - 1].x, re.x), fma(C[m], a[k - 1].y, re.y));
+                im = mk(fma(S[m], b[k - 1].x, im.x), fma(S[m], b[k - 1].y, im.y));
+            }
+            const cplx t = mul_w4<INV>(im);              // -i im (forward), +i im (inverse)
+            out[s] = cadd(re, t);
+            out[R - s] = csub(re, t);
+        }
+#pragma unroll
+        for (int s = 0; s < R; ++s) v[s] = out[s];
+    }
+};
+
+template <bool INV>
+struct Butterfly<5, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[5])
+    {
+        // cos, sin of 2 pi m/5
+        const double C[5] = {1.0, 0.30901699437494742410229341718282, -0.80901699437494742410229341718282,
+                             -0.80901699437494742410229341718282, 0.30901699437494742410229341718282};
+        const double S[5] = {0.0, 0.95105651629515357211643933337938, 0.58778525229247312916870595463907,
+                             -0.58778525229247312916870595463907, -0.95105651629515357211643933337938};
+        OddPrimeButterfly<5, INV>::run(v, C, S);
+    }
+};
+
+template <bool INV>
+struct Butterfly<7, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[7])
+    {
+        // cos, sin of 2 pi m/7
+        const double C[7] = {1.0, 0.62348980185873353052500488400424, -0.22252093395631440428890256449679,
+                             -0.90096886790241912623610231950745, -0.90096886790241912623610231950745,
+                             -0.22252093395631440428890256449679, 0.62348980185873353052500488400424};
+        const double S[7] = {0.0, 0.78183148246802980870844452667406, 0.97492791218182360701813168299393,
+                             0.43388373911755812047576833284836, -0.43388373911755812047576833284836,
+                             -0.97492791218182360701813168299393, -0.78183148246802980870844452667406};
+        OddPrimeButterfly<7, INV>::run(v, C, S);
     }
 };
 
@@ -166,6 +231,10 @@ __device__ __forceinline__ void fft_run(const FftPlan& P, int b, bool active,
             DGPE_PASS(2, 2)
             DGPE_PASS(2, 3)
             DGPE_PASS(2, 4)
+            DGPE_PASS(5, 1)
+            DGPE_PASS(5, 2)
+            DGPE_PASS(7, 1)
+            DGPE_PASS(7, 2)
             default: break;
         }
 #undef DGPE_PASS

@@ -44,11 +44,12 @@ struct ZGeom {
     static constexpr int M = NZ / 2;
     static constexpr int T = z_team(NZ);                       // lanes per line
     static constexpr int LPW = 32 / T;                         // lines per warp
-    static constexpr int NPER = NZ / T;                        // psi elements per lane (coalesced walks)
+    static constexpr int NPER = (NZ + T - 1) / T;              // psi elements per lane (coalesced walks)
+    static constexpr int KPER = (M + T - 1) / T;               // spectrum bins per lane
     static constexpr int LC = ((NZ - 2 + T - 1) / T) | 1;      // sweep chunk per lane, odd
     static constexpr int A_ELEMS = NZ;
     static constexpr int B_ELEMS = (M + (M >> 3) + 7) / 8 * 8;
-    static_assert(NZ % 64 == 0, "z-line kernels need nz to be a multiple of 64");
+    static_assert(NZ % 2 == 0 && NZ >= 32, "z-line kernels need an even nz >= 32");
 };
 
 struct PosPad {
@@ -96,7 +97,7 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
     // z_m, m = lane + TL q, is exactly what butterfly `lane` of the first pass reads when that pass has
     // radix M/TL: then each lane loads its pairs (psi_{2m}, psi_{2m+1}) with one 256-bit load -- a warp
     // reads 1 KB contiguous -- and the densities go from registers straight into the pass
-    constexpr bool FIRST_IN_REGS = (ct::radix_at(M, 0, false) == M / TL);
+    constexpr bool FIRST_IN_REGS = (M % TL == 0) && (ct::radix_at(M, 0, false) == M / TL);
     if constexpr (FIRST_IN_REGS) {
         using P0 = CtPass<M, 0, false, false, TL>;
         static_assert(P0::NB == 1 && P0::R == M / TL && P0::Ns == 1, "first pass must be one butterfly per lane");
@@ -123,11 +124,14 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
     } else {
         cplx a[G::NPER];
 #pragma unroll
-        for (int i = 0; i < G::NPER; ++i) a[i] = ld_stream(p + TL * i + lane);
+        for (int i = 0; i < G::NPER; ++i) {
+            const int e = TL * i + lane;
+            a[i] = (NZ % TL == 0 || e < NZ) ? ld_stream(p + e) : mk(0.0, 0.0);
+        }
 #pragma unroll
         for (int i = 0; i < G::NPER; ++i) {
             const int e = TL * i + lane, m = e >> 1;
-            Bd[2 * PosPad::at(m) + (e & 1)] = s2 * cabs2(a[i]);
+            if (NZ % TL == 0 || e < NZ) Bd[2 * PosPad::at(m) + (e & 1)] = s2 * cabs2(a[i]);
         }
         __syncwarp();
         ct_fft_range<M, false, false, TL, SyncWarp, PosPad, 0, L, false>(B, lane, true, tw, none, keep);
@@ -145,7 +149,8 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
         if (valid) st_stream(out + k, mk(0.5 * (s.x + wd.y), 0.5 * (s.y - wd.x)));     // s/2 - (i/2) w d
     };
 #pragma unroll
-    for (int t = 0; t < M / TL; ++t) split(lane + TL * t);
+    for (int t = 0; t < G::KPER; ++t)
+        if (M % TL == 0 || lane + TL * t < M) split(lane + TL * t);
     if (lane == 0) split(M);
 }
 
@@ -242,18 +247,18 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         // ---- Hermitian merge straight from global memory ----
         // Z_k, k = lane + TL t, is exactly what butterfly `lane` of the first inverse pass reads when that
         // pass has radix M/TL: then the merged values go from registers straight into the pass
-        constexpr bool FIRST_IN_REGS = (ct::radix_at(M, 0, false) == M / TL);
+        constexpr bool FIRST_IN_REGS = (M % TL == 0) && (ct::radix_at(M, 0, false) == M / TL);
         const cplx* in = spec + (long long)line * (M + 1);
-        cplx xa[M / TL], xb[M / TL];
+        cplx xa[G::KPER], xb[G::KPER];
 #pragma unroll
-        for (int t = 0; t < M / TL; ++t) {
-            const int k = lane + TL * t;
+        for (int t = 0; t < G::KPER; ++t) {
+            const int k = min(lane + TL * t, M - 1);              // (bins past M-1: loaded twice, never stored)
             xa[t] = ld_stream(in + k);
             xb[t] = ld_stream(in + (M - k));
         }
 #pragma unroll
-        for (int t = 0; t < M / TL; ++t) {
-            const int k = lane + TL * t;
+        for (int t = 0; t < G::KPER; ++t) {
+            const int k = min(lane + TL * t, M - 1);
             const cplx w = cconj(__ldg(&Z.tws[k]));               // e^{+2 pi i k/nz}
             const cplx cb = cconj(xb[t]);
             const cplx s = cadd(xa[t], cb), d = csub(xa[t], cb);
@@ -282,7 +287,8 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
             }
         } else {
 #pragma unroll
-            for (int t = 0; t < M / TL; ++t) B[PosPad::at(lane + TL * t)] = xa[t];
+            for (int t = 0; t < G::KPER; ++t)
+                if (M % TL == 0 || lane + TL * t < M) B[PosPad::at(lane + TL * t)] = xa[t];
             __syncwarp();
             ct_fft_range<M, true, false, TL, SyncWarp, PosPad, 0, L, false>(B, lane, true, Z.tw, none, keep_phi);
         }

@@ -39,7 +39,11 @@ def pair(gpu, oracle, shape, d, dt, trap, g, gdd, mode):
 # (the last three: the 768- and 384-point kernels of BJ:configs[4] -- TMA-fed sweeps with 96 chunks per line,
 # four-pass FFTs with a radix-3 pass, the 384-point z-line kernels -- on thin boxes the oracle finishes fast)
 STAGE_SHAPES = [(4, 4, 4), (8, 8, 8), (6, 9, 12), (12, 18, 16), (27, 32, 6), (16, 24, 36), (64, 64, 64),
-                (48, 96, 128), (9, 4, 18), (768, 8, 64), (16, 768, 128), (8, 384, 384)]
+                (48, 96, 128), (9, 4, 18), (768, 8, 64), (16, 768, 128), (8, 384, 384),
+                # radix 5 and 7 (SV section 8f NEXT-1): generic plans, and the specialised 160/240/480/500
+                # lengths of the paper's own grids (480^3, 480x480x500, 480x480x250: P:L75, L96, L111)
+                (10, 14, 20), (35, 25, 50), (7, 5, 98), (480, 8, 70), (8, 500, 250), (16, 240, 160), (8, 160, 320),
+                (8, 8, 480), (12, 8, 500), (8, 8, 640), (8, 12, 240)]
 
 
 @pytest.mark.parametrize("shape", STAGE_SHAPES)
