@@ -46,8 +46,10 @@ def parse():
 def workload_name(cfg):
     nx, ny, nz = cfg.shape
     mode = "imaginary-time" if cfg.mode == 0 else "real-time"
+    src = (f"BASELINE.json configs[{int(cfg.name[1]) - 1}]" if cfg.name[0] == "C" else
+           "grid of the paper's timing table " + cfg.name[1] + ", physics borrowed from C4: context only")
     return (f"{cfg.name}: {mode} dipolar GPE {nx}x{ny}x{nz} fp64 complex, dx={cfg.d[0]} dt={cfg.dt} "
-            f"trap={cfg.trap} g={cfg.g} gdd={cfg.gdd} (BASELINE.json configs[{int(cfg.name[1]) - 1}])")
+            f"trap={cfg.trap} g={cfg.g} gdd={cfg.gdd} ({src})")
 
 
 def load_peaks():

@@ -69,6 +69,17 @@ CONFIGS = {
 }
 
 
+# The grids of the paper's own timing tables (Table 1: 480^3; Table 2: 480x480x500; P:L111
+# Table 3: 480x480x250), for like-for-like CONTEXT runs only (`bench.py --config T1i` ...).  The paper
+# does not state the physics of those runs, so they borrow C4's spacings, time step, trap
+# and interaction strengths; timing is data-independent.  i = imaginary time, r = real time.
+PAPER_GRIDS = {"T1": (480, 480, 480), "T2": (480, 480, 500), "T3": (480, 480, 250)}
+for _k, _shape in PAPER_GRIDS.items():
+    for _m, _mode in (("i", IMAG), ("r", REAL)):
+        CONFIGS[_k + _m] = Config(_k + _m, _shape, (0.1,) * 3, 0.002, (1.0, 1.0, 4.0), 300.0, 200.0, _mode, 1000, 4,
+                                  (1.0, 1.0, 4.0))
+
+
 def scaled(cfg: Config, shape, name=None) -> Config:
     """Same physics on a smaller grid (same spacings): for parity cases the oracle finishes quickly."""
     return replace(cfg, shape=tuple(shape), name=name or f"{cfg.name}@{'x'.join(map(str, shape))}",
