@@ -499,18 +499,20 @@ static void fill_chunk_tabs(const AxisSweep& S, bool use, ChunkTabs<CT, LC>* P)
     }
 }
 
+constexpr int Z_MAIN_WARPS = 1;      // warps per CTA of k_z_main: one, so that a finished line frees its slot at once
+
 template <int NZ>
 constexpr int z_main_minb(bool use_a, bool use_b)
 {
-    const int per_cta = 4 * ZGeom<NZ>::LPW * ((use_a ? ZGeom<NZ>::A_ELEMS : 0) + (use_b ? ZGeom<NZ>::B_ELEMS : 0)) * 16 + 1024;
-    const int m = (227 * 1024) / per_cta;
-    return m < 1 ? 1 : (m > 4 ? 4 : m);
+    const int per_cta = Z_MAIN_WARPS * ZGeom<NZ>::LPW * ((use_a ? ZGeom<NZ>::A_ELEMS : 0) + (use_b ? ZGeom<NZ>::B_ELEMS : 0)) * 16 + 1024;
+    const int m = (227 * 1024) / per_cta, cap = 16 / Z_MAIN_WARPS;       // 16 warps per SM: 128 registers per thread
+    return m < 1 ? 1 : (m > cap ? cap : m);
 }
 
 template <int NZ>
 static int launch_z_r2c_n(dgpe_handle* h, const cplx* psi)
 {
-    constexpr int WARPS = 8;
+    constexpr int WARPS = 1;                             // one warp per CTA: a finished line frees its slot at once
     constexpr int LINES = WARPS * ZGeom<NZ>::LPW;        // lines per CTA
     const size_t smem = (size_t)LINES * ZGeom<NZ>::B_ELEMS * sizeof(cplx);
     auto kern = k_z_r2c<NZ, WARPS>;
@@ -527,7 +529,7 @@ static int launch_z_r2c_n(dgpe_handle* h, const cplx* psi)
 template <int NZ, typename CT, int SPEC, bool SWEEP, bool CONSTTAB>
 static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
 {
-    constexpr int WARPS = 4, LC = ZGeom<NZ>::LC, LINES = WARPS * ZGeom<NZ>::LPW;
+    constexpr int WARPS = Z_MAIN_WARPS, LC = ZGeom<NZ>::LC, LINES = WARPS * ZGeom<NZ>::LPW;
     constexpr bool USE_A = SPEC != ZS_PHI, USE_B = SPEC != ZS_NONE;
     constexpr int MINB = z_main_minb<NZ>(USE_A, USE_B);
     const size_t smem = (size_t)LINES * ((USE_A ? ZGeom<NZ>::A_ELEMS : 0) + (USE_B ? ZGeom<NZ>::B_ELEMS : 0)) * sizeof(cplx);
