@@ -22,6 +22,7 @@
 #include "xyfft.cuh"
 #include "xysweep.cuh"
 #include "xysweep_tma.cuh"
+#include "xyfft_tma.cuh"
 #include "zline.cuh"
 
 using namespace dgpe;
@@ -79,6 +80,7 @@ struct dgpe_handle {
     // L2 prefetch of the next residency, per kernel family (DGPE_PREFETCH=<mask> overrides, for A/B runs):
     // it pays for the z-line kernels and the y axis; on the x axis (row stride ny*nz) it costs time
     int prefetch = PF_Z | PF_SWEEP_Y | PF_FFT_Y;
+    bool use_tma_fft = true;         // DGPE_TMA_FFT=0: K2/K4 load and store through the threads (k_fft_xy)
     bool use_tma_x = false;          // DGPE_TMA=2: TMA on the x axis at every length (A/B)
     bool use_tma = true;             // DGPE_TMA=0: the x/y sweeps load and store through the threads (k_sweep_xy)
     bool zfast = false;              // warp-per-line z kernels (zline.cuh) and the fused step order z, x, y
@@ -302,6 +304,8 @@ static int init_handle(dgpe_handle* h)
         const char* tm = getenv("DGPE_TMA");
         h->use_tma = !(tm && tm[0] == '0');
         h->use_tma_x = tm && tm[0] == '2';
+        const char* tf = getenv("DGPE_TMA_FFT");
+        h->use_tma_fft = h->use_tma && !(tf && tf[0] == '0');
         const char* gr = getenv("DGPE_GRAPH");
         h->use_graph = !(gr && gr[0] == '0');
         const char* pm = getenv("DGPE_PF_MULT");
@@ -669,12 +673,90 @@ static int launch_fft_xy(dgpe_handle* h, int n, const LineMap& map, int nbatch, 
     }
 }
 
+// cuTensorMapEncodeTiled through the runtime (no link against libcuda)
+static PFN_cuTensorMapEncodeTiled_v12000 tensor_map_encoder()
+{
+    static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (PFN_cuTensorMapEncodeTiled_v12000)p;
+        cudaGetLastError();
+    }
+    return fn;
+}
+
+
+// number of equal TMA boxes (<= 256 rows each) a line of n rows splits into; 0 if none
+static constexpr int tma_boxes(int n)
+{
+    for (int k = (n + 255) / 256; k <= 8; ++k)
+        if (n % k == 0 && n / k <= 256) return k;
+    return 0;
+}
+
+// ---- K2 / K4 on the TMA pipeline (xyfft_tma.cuh): the long y lines ----
+template <int N, bool INV, int NSTAGE>
+static int launch_fft_tma_s(dgpe_handle* h)
+{
+    auto kern = k_fft_tma<N, INV, NSTAGE>;
+    const size_t smem = (size_t)NSTAGE * N * TILE_COLS * sizeof(cplx) + 128;
+    static bool ready = false;
+    if (!ready) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ready = true;
+    }
+    const cuuint64_t nx = h->nx, ny = h->ny, nzh = h->nzh;
+    constexpr int nbox = tma_boxes(N);
+    static_assert(nbox > 0 && N % nbox == 0 && N / nbox <= 256, "line length must split into equal TMA boxes");
+    cuuint64_t dims[3] = {2 * nzh, ny, nx}, strides[2] = {nzh * 16, ny * nzh * 16};
+    cuuint32_t box[3] = {2 * TILE_COLS, (cuuint32_t)(N / nbox), 1}, estr[3] = {1, 1, 1};
+    CUtensorMap tmap;
+    CUresult cr = tensor_map_encoder()(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, h->spec, dims, strides, box, estr,
+                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                       CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (cr != CUDA_SUCCESS) return fail(DGPE_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)cr);
+    TmaWalk W;
+    W.n = N; W.box_rows = N / nbox;
+    W.tiles_per_batch = (h->nzh + TILE_COLS - 1) / TILE_COLS;
+    W.ntiles = W.tiles_per_batch * h->nx;
+    kern<<<std::min(W.ntiles, h->num_sms), xy_threads<N>(), smem, h->stream>>>(tmap, W, h->tw_y);
+    return check_launch("k_fft_tma");
+}
+
+template <int N>
+static int launch_fft_tma_n(dgpe_handle* h, bool inverse)
+{
+    constexpr int NSTAGE = (3 * N * 128 <= 200 * 1024) ? 3 : 2;
+    return inverse ? launch_fft_tma_s<N, true, NSTAGE>(h) : launch_fft_tma_s<N, false, NSTAGE>(h);
+}
+
+static int launch_fft_tma(dgpe_handle* h, bool inverse, bool* handled)
+{
+    *handled = h->use_tma_fft && tensor_map_encoder() != nullptr;
+    if (!*handled) return DGPE_OK;
+    switch (h->ny) {
+        case 384: return launch_fft_tma_n<384>(h, inverse);
+        case 480: return launch_fft_tma_n<480>(h, inverse);
+        case 512: return launch_fft_tma_n<512>(h, inverse);
+        case 640: return launch_fft_tma_n<640>(h, inverse);
+        case 768: return launch_fft_tma_n<768>(h, inverse);
+        default: *handled = false; return DGPE_OK;
+    }
+}
+
 static int launch_fft_y(dgpe_handle* h, bool inverse)
 {
     const int nx = h->nx, ny = h->ny, nzh = h->nzh;
     LineMap my{ny, nzh, (long long)ny * nzh, 1, nzh};
     if (!h->force_generic) {
         bool handled = false;
+        int rct = launch_fft_tma(h, inverse, &handled);
+        if (rct || handled) return rct;
         int rc = inverse ? launch_fft_xy<FFT_INV>(h, ny, my, nx, h->tw_y, &handled)
                          : launch_fft_xy<FFT_FWD>(h, ny, my, nx, h->tw_y, &handled);
         if (rc || handled) return rc;
@@ -744,29 +826,13 @@ static int launch_c2r(dgpe_handle* h, cplx* psi, int kmode, double* out)
 }
 
 // ---- TMA-fed persistent sweep (xysweep_tma.cuh) ----
-static PFN_cuTensorMapEncodeTiled_v12000 tensor_map_encoder()
-{
-    static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = (PFN_cuTensorMapEncodeTiled_v12000)p;
-        cudaGetLastError();
-    }
-    return fn;
-}
-
 // can the TMA kernel take this sweep?  (whole tiles, a tile stage count >= 2 in shared memory, boxes <= 256 rows)
 static bool tma_sweep_ok(const dgpe_handle* h, const LineMap& m, const AxisSweep& S, int* box_rows, int* nstage)
 {
     if (!h->use_tma || h->force_generic || S.Lc != TMA_LC || S.G > 96 || m.ncols % TILE_COLS) return false;
     if (!tensor_map_encoder()) return false;
-    const int nbox = (m.n + 255) / 256;
-    if (m.n % nbox) return false;
+    const int nbox = tma_boxes(m.n);
+    if (!nbox) return false;
     const size_t tile = (size_t)m.n * TILE_COLS * sizeof(cplx);
     int ns = (int)((200 * 1024) / tile);
     if (ns < 2) return false;

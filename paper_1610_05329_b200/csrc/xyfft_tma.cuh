@@ -1,0 +1,96 @@
+// xyfft_tma.cuh -- K2 / K4 (FFT of the half-spectrum along y) as a persistent, TMA-fed pipeline.
+//
+// Same passes as k_fft_xy (xyfft.cuh, ctfft.cuh); what changes is how the tile moves, exactly as in
+// xysweep_tma.cuh: one CTA per SM walks the tiles, the Tensor Memory Accelerator fetches tile i+1 (and
+// i+2) into another shared-memory stage while the CTA transforms tile i in place, and the result leaves
+// by a TMA tensor store from the same stage.  The rows of a tile start at multiples of 16 bytes only
+// (nz/2+1 is odd), which the TMA does not mind, and the ragged last tile of a row (one valid kz bin out
+// of 8 at nz/2+1 = 257) is zero-filled on load and clipped on store by the tensor map bounds.
+//
+// Tensor map (host): rank 3 over the half-spectrum viewed as doubles, {2 (nz/2+1), ny, nx}; a tile is
+// the box {16 doubles, rows, 1}.
+#pragma once
+#include "xyfft.cuh"
+#include "xysweep_tma.cuh"
+
+namespace dgpe {
+
+// grid = min(ntiles, #SMs); block = xy_threads<N>(); dynamic smem = NSTAGE * N * 128 bytes (+128)
+template <int N, bool INV, int NSTAGE>
+__global__ void __launch_bounds__(xy_threads<N>(), 1)
+k_fft_tma(const __grid_constant__ CUtensorMap tmap, TmaWalk W, const cplx* __restrict__ tw)
+{
+    constexpr int NBF = xy_nbf<N>();
+    constexpr int L = ct::npass(N);
+    static_assert(L >= 2, "the pipelined kernel is for the long lines");
+    extern __shared__ unsigned char smem_dyn[];
+    __shared__ __align__(8) unsigned long long full[NSTAGE];
+    cplx* stages = reinterpret_cast<cplx*>((reinterpret_cast<uintptr_t>(smem_dyn) + 127) & ~uintptr_t(127));
+    constexpr int tile_elems = N * TILE_COLS;
+    constexpr unsigned tile_bytes = (unsigned)tile_elems * 16u;
+    const int tid = threadIdx.x, c = tid & 7, b = tid >> 3;
+    const bool on = b < NBF;
+    const int first = blockIdx.x, stride = gridDim.x;
+    const int nmine = (first < W.ntiles) ? (W.ntiles - first + stride - 1) / stride : 0;
+
+    auto coords = [&](int it, int& c0, int& c2) {
+        const int t = first + it * stride;
+        const int bat = t / W.tiles_per_batch;
+        c0 = (t - bat * W.tiles_per_batch) * (2 * TILE_COLS);
+        c2 = bat;
+    };
+    auto issue_load = [&](int it) {                     // thread 0 only
+        int c0, c2;
+        coords(it, c0, c2);
+        const int st = it % NSTAGE;
+        mbar_expect_tx(&full[st], tile_bytes);
+        for (int r0 = 0; r0 < N; r0 += W.box_rows)
+            tma_load_3d(stages + (size_t)st * tile_elems + (size_t)r0 * TILE_COLS, &tmap, c0, r0, c2, &full[st]);
+    };
+
+    if (tid == 0) {
+        for (int st = 0; st < NSTAGE; ++st) mbar_init(&full[st], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0)
+        for (int it = 0; it < NSTAGE - 1 && it < nmine; ++it) issue_load(it);
+
+    for (int it = 0; it < nmine; ++it) {
+        const int st = it % NSTAGE;
+        cplx* tile = stages + (size_t)st * tile_elems;
+        cplx* col = tile + c;
+        mbar_wait(&full[st], (unsigned)((it / NSTAGE) & 1));
+
+        // pass 0 by hand, so that the refill of the stage tile it-1 used can be issued after its barrier
+        CtPass<N, 0, INV, false, NBF> p0;
+        if (on) p0.load(b, [&](int idx) { return col[PosTile::at(idx)]; });
+        __syncthreads();                                 // every read of pass 0 precedes its writes
+        if (tid == 0 && it + NSTAGE - 1 < nmine) {
+            tma_store_wait_read<0>();                    // the store of tile it-1 has read its stage
+            issue_load(it + NSTAGE - 1);
+        }
+        if (on) {
+            p0.bfly(b);
+            p0.scatter(b, [&](int idx, cplx val) { col[PosTile::at(idx)] = val; });
+        }
+        CtPass<N, 1, INV, false, NBF> p1;
+        if (on) p1.load_tw(b, tw);                       // overlaps the barrier wait
+        __syncthreads();
+        auto none = [](int) { return mk(0.0, 0.0); };
+        ct_fft_range_tw<N, INV, false, NBF, SyncCta, PosTile, 1, L, false>(
+            p1, col, b, on, tw, none, [&](int idx, cplx val) { col[PosTile::at(idx)] = val; });
+
+        fence_proxy_async();                             // my tile writes -> visible to the TMA store
+        __syncthreads();
+        if (tid == 0) {
+            int c0, c2;
+            coords(it, c0, c2);
+            for (int r0 = 0; r0 < N; r0 += W.box_rows) tma_store_3d(&tmap, c0, r0, c2, tile + (size_t)r0 * TILE_COLS);
+            tma_store_commit();
+        }
+    }
+    if (tid == 0) tma_store_wait<0>();
+}
+
+}  // namespace dgpe
