@@ -10,6 +10,10 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <mutex>
+#include <tuple>
+#include <utility>
 #include <vector>
 
 #include <cudaTypedefs.h>
@@ -285,6 +289,31 @@ static int allow_smem(K kernel, size_t bytes)
     return DGPE_OK;
 }
 
+// Per (kernel, device) setup that must precede a launch with more than 48 KB of dynamic shared memory,
+// and the resident CTAs per SM of that launch shape.  Cached: the kernels are launched thousands of
+// times; keyed by device so that one process may hold handles on several GPUs; guarded for threads.
+static int kernel_setup(const void* func, int threads, size_t smem, int* ctas_per_sm)
+{
+    static std::mutex mu;
+    static std::map<std::pair<const void*, int>, size_t> allowed;                              // (kernel, device) -> opt-in bytes
+    static std::map<std::tuple<const void*, int, int, size_t>, int> resident;                  // + (threads, bytes) -> CTAs per SM
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(mu);
+    size_t& optin = allowed[std::make_pair(func, dev)];
+    if (smem > 48 * 1024 && smem > optin) {
+        CU(cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        optin = smem;
+    }
+    int& n = resident[std::make_tuple(func, dev, threads, smem)];
+    if (!n) {
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, func, threads, smem));
+        if (n < 1) return fail(DGPE_ERR_CUDA, "a kernel does not fit on an SM (%d threads, %zu bytes of shared memory)", threads, smem);
+    }
+    if (ctas_per_sm) *ctas_per_sm = n;
+    return DGPE_OK;
+}
+
 static int init_handle(dgpe_handle* h)
 {
     const int nx = h->nx, ny = h->ny, nz = h->nz, nzh = h->nzh, M = nz / 2;
@@ -520,11 +549,8 @@ static int launch_z_r2c_n(dgpe_handle* h, const cplx* psi)
     constexpr int LINES = WARPS * ZGeom<NZ>::LPW;        // lines per CTA
     const size_t smem = (size_t)LINES * ZGeom<NZ>::B_ELEMS * sizeof(cplx);
     auto kern = k_z_r2c<NZ, WARPS>;
-    static bool ready = false;
-    if (!ready) {
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        ready = true;
-    }
+    int rc = kernel_setup((const void*)kern, 32 * WARPS, smem, nullptr);
+    if (rc) return rc;
     const int nlines = h->nx * h->ny;
     kern<<<(nlines + LINES - 1) / LINES, 32 * WARPS, smem, h->stream>>>(psi, h->spec, nlines, h->tw_zh, h->tw_split, h->scal);
     return check_launch("k_z_r2c");
@@ -538,11 +564,9 @@ static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
     constexpr int MINB = z_main_minb<NZ>(USE_A, USE_B);
     const size_t smem = (size_t)LINES * ((USE_A ? ZGeom<NZ>::A_ELEMS : 0) + (USE_B ? ZGeom<NZ>::B_ELEMS : 0)) * sizeof(cplx);
     auto kern = k_z_main<NZ, CT, SPEC, SWEEP, CONSTTAB, WARPS, MINB>;
-    static bool ready = false;
-    if (!ready) {
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        ready = true;
-    }
+    int ctas_per_sm = 0;
+    int rc = kernel_setup((const void*)kern, 32 * WARPS, smem, &ctas_per_sm);
+    if (rc) return rc;
     const AxisSweep& S = h->sw[2];
     SweepTables<CT> T;
     T.r = to_ct<CT>(S.r);
@@ -559,11 +583,7 @@ static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
     Z.vx = h->vx; Z.vy = h->vy;
     Z.dz = h->dz; Z.lam2 = h->lambda * h->lambda;
     Z.scal = h->scal; Z.tw = h->tw_zh; Z.tws = h->tw_split; Z.phi_out = phi_out;
-    {
-        static int ctas_per_sm = 0;
-        if (!ctas_per_sm) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, 32 * WARPS, smem));
-        Z.pf_lines = (h->prefetch & PF_Z) ? h->pf_mult * ctas_per_sm * h->num_sms * LINES : 0;
-    }
+    Z.pf_lines = (h->prefetch & PF_Z) ? h->pf_mult * ctas_per_sm * h->num_sms * LINES : 0;
     kern<<<(Z.nlines + LINES - 1) / LINES, 32 * WARPS, smem, h->stream>>>(psi, h->spec, Z, T, P);
     return check_launch("k_z_main");
 }
@@ -630,13 +650,9 @@ static int launch_fft_xy_n(dgpe_handle* h, const LineMap& map, int nbatch, const
 {
     const size_t smem = (size_t)N * TILE_COLS * sizeof(cplx);
     auto kern = k_fft_xy<N, KIND>;
-    static bool ready = false;           // per instantiation (one device per process)
-    if (!ready) {
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        ready = true;
-    }
-    static int ctas_per_sm = 0;
-    if (!ctas_per_sm) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, xy_threads<N>(), smem));
+    int ctas_per_sm = 0;
+    int rc = kernel_setup((const void*)kern, xy_threads<N>(), smem, &ctas_per_sm);
+    if (rc) return rc;
     UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 1.0 / (double)h->N,
               (h->prefetch & (KIND == FFT_X_UDD ? PF_FFT_X : PF_FFT_Y)) ? h->pf_mult * ctas_per_sm * h->num_sms : 0};
     dim3 grid((map.ncols + TILE_COLS - 1) / TILE_COLS, nbatch);
@@ -705,11 +721,8 @@ static int launch_fft_tma_s(dgpe_handle* h)
 {
     auto kern = k_fft_tma<N, INV, NSTAGE>;
     const size_t smem = (size_t)NSTAGE * N * TILE_COLS * sizeof(cplx) + 128;
-    static bool ready = false;
-    if (!ready) {
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        ready = true;
-    }
+    int rc = kernel_setup((const void*)kern, xy_threads<N>(), smem, nullptr);
+    if (rc) return rc;
     const cuuint64_t nx = h->nx, ny = h->ny, nzh = h->nzh;
     constexpr int nbox = tma_boxes(N);
     static_assert(nbox > 0 && N % nbox == 0 && N / nbox <= 256, "line length must split into equal TMA boxes");
@@ -850,14 +863,9 @@ static int launch_sweep_tma_s(dgpe_handle* h, cplx* psi, int axis, const LineMap
 {
     auto kern = k_sweep_tma<CT, CONSTTAB, NSTAGE, NTMAX>;
     const size_t smem = (size_t)NSTAGE * m.n * TILE_COLS * sizeof(cplx) + 128;
-    static size_t allowed = 0;
-    if (smem > allowed) {
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        allowed = smem;
-    }
     int ctas_per_sm = 1;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, thr, smem));
-    if (ctas_per_sm < 1) return fail(DGPE_ERR_CUDA, "k_sweep_tma does not fit on an SM (n = %d)", m.n);
+    int rc = kernel_setup((const void*)kern, thr, smem, &ctas_per_sm);
+    if (rc) return rc;
     // psi viewed as doubles: x sweep {2 ny nz, nx, 1}, y sweep {2 nz, ny, nx}; box {16, box_rows, 1}
     const cuuint64_t nx = h->nx, ny = h->ny, nz = h->nz;
     cuuint64_t dims[3], strides[2];
@@ -902,7 +910,8 @@ static int launch_sweep_xy(dgpe_handle* h, cplx* psi, const LineMap& m, dim3 gri
     ChunkTabs<CT, LC> P;
     fill_chunk_tabs<CT, LC>(S, CONSTTAB, &P);
     int ctas_per_sm = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, thr, 0));
+    int rc = kernel_setup((const void*)kern, thr, 0, &ctas_per_sm);
+    if (rc) return rc;
     const int pf = (h->prefetch & (m.batch_stride ? PF_SWEEP_Y : PF_SWEEP_X)) ? h->pf_mult * ctas_per_sm * h->num_sms : 0;
     kern<<<grid, thr, 0, h->stream>>>(psi, m, T, F, pf, P);
     return check_launch("k_sweep_xy");
