@@ -142,7 +142,7 @@ static bool smooth2357(int n)
 }
 
 // radices 8, 4, 2 first, then 3, 5, 7; butterfly slots per column = n / largest radix
-static int make_plan(dgpe_handle* h, int n, FftPlan* P, cplx** tw_dev)
+static int make_plan(dgpe_handle* h, int n, FftPlan* P, cplx** tw_dev, int max_slots)
 {
     std::memset(P, 0, sizeof(*P));
     P->n = n;
@@ -162,7 +162,7 @@ static int make_plan(dgpe_handle* h, int n, FftPlan* P, cplx** tw_dev)
         return fail(DGPE_ERR_ARG, "FFT length %d too small", n);
     }
     P->npass = np;
-    P->nbf = n / rmax;
+    P->nbf = std::min(n / rmax, max_slots);      // 8 * nbf threads per tile, bounded by the kernel (then a slot runs several butterflies)
     for (int p = 0; p < np; ++p) {
         const int nbut = n / P->radix[p];
         P->nb[p] = (nbut + P->nbf - 1) / P->nbf;
@@ -341,9 +341,9 @@ static int init_handle(dgpe_handle* h)
         if (pm && atoi(pm) > 0) h->pf_mult = atoi(pm);
     }
 
-    if ((rc = make_plan(h, nx, &h->plan_x, &h->tw_x))) return rc;
-    if ((rc = make_plan(h, ny, &h->plan_y, &h->tw_y))) return rc;
-    if ((rc = make_plan(h, M, &h->plan_zh, &h->tw_zh))) return rc;
+    if ((rc = make_plan(h, nx, &h->plan_x, &h->tw_x, 128))) return rc;
+    if ((rc = make_plan(h, ny, &h->plan_y, &h->tw_y, 128))) return rc;
+    if ((rc = make_plan(h, M, &h->plan_zh, &h->tw_zh, 64))) return rc;
     {
         std::vector<cplx> tw(M + 1);
         const long double TWO_PI = 6.283185307179586476925286766559005768L;
@@ -379,6 +379,7 @@ static int init_handle(dgpe_handle* h)
         // chunk length of the sweep recursions: 8 (or 16) unknowns per thread on the strided axes; on z
         // the warp-per-line kernel gives every lane ceil((nz-2)/32) unknowns
         int lc = (ns[a] <= 770 && !h->force_generic) ? 8 : 16;
+        if (a == 2 && !h->zfast) lc = 16;      // generic z kernel: 8 * G <= 512 threads
         if (a == 2 && h->zfast) lc = ((nz - 2 + z_team(nz) - 1) / z_team(nz)) | 1;      // = ZGeom<nz>::LC, odd (zline.cuh)
         if (h->mode == DGPE_IMAG)
             rc = build_sweep<double>(h, &h->sw[a], ns[a], std::complex<double>(rr, 0.0), lc);

@@ -43,7 +43,9 @@ STAGE_SHAPES = [(4, 4, 4), (8, 8, 8), (6, 9, 12), (12, 18, 16), (27, 32, 6), (16
                 # radix 5 and 7 (SV section 8f NEXT-1): generic plans, and the specialised 160/240/480/500
                 # lengths of the paper's own grids (480^3, 480x480x500, 480x480x250: P:L75, L96, L111)
                 (10, 14, 20), (35, 25, 50), (7, 5, 98), (480, 8, 70), (8, 500, 250), (16, 240, 160), (8, 160, 320),
-                (8, 8, 480), (12, 8, 500), (8, 8, 640), (8, 12, 240)]
+                (8, 8, 480), (12, 8, 500), (8, 8, 640), (8, 12, 240),
+                # lengths whose largest radix is small (more than 128 butterflies per pass: several per thread)
+                (486, 4, 6), (4, 729, 4), (4, 6, 972), (686, 4, 10), (4, 6, 600)]
 
 
 @pytest.mark.parametrize("shape", STAGE_SHAPES)
