@@ -98,6 +98,41 @@ def test_sweeps_with_large_r_need_the_long_lookback(gpu, oracle, mode, dt):
             assert np.max(np.abs(t.cpu().numpy() - a)) <= 1e-12 * (1 + dt), (shape, axis)
 
 
+def _smooth_lengths(lo=4, hi=1024):
+    out = []
+    for n in range(lo, hi + 1):
+        m = n
+        for f in (2, 3, 5, 7):
+            while m % f == 0:
+                m //= f
+        if m == 1:
+            out.append(n)
+    return out
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_every_supported_length_on_every_axis(gpu, oracle, axis, mode):
+    """One full step (imaginary or real time) for EVERY length 2^a 3^b 5^c 7^d in [4, 1024] on each axis (thin box in
+    the other two), against the oracle: every plan, specialised or generic, launches and is right."""
+    worst = 0.0
+    for n in _smooth_lengths():
+        if axis == 2 and n % 2:
+            continue
+        shape = [8, 8, 8]
+        shape[axis] = n
+        shape = tuple(shape)
+        G, O = pair(gpu, oracle, shape, (0.3, 0.25, 0.2), 0.01, (1.0, 0.7, 1.3), 5.0, 3.0, mode)
+        psi = inputs.random_state(shape, 100 + n) * 0.3
+        t, a = dev(psi), psi.copy()
+        assert G.step(t, 1) == O.step(a, 1) == 0, shape
+        err = float(np.max(np.abs(t.cpu().numpy() - a)))
+        assert err <= TOL_1, (shape, err)
+        worst = max(worst, err)
+        G.close()
+    print(f"mode {mode} axis {axis}: worst |dpsi| over all lengths = {worst:.2e}")
+
+
 def run_both(gpu, oracle, cfg, checkpoints, psi0=None):
     """Step GPU and oracle side by side; at each checkpoint return (step, max|dpsi|, obs_gpu, obs_ref)."""
     psi0 = inputs.initial_state(cfg) if psi0 is None else psi0
