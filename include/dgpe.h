@@ -55,8 +55,8 @@ enum {
 
 /*
  * dgpe_create -- build a handle for one grid and one set of physical parameters.
- *   nx, ny, nz   grid points per axis; each >= 4, of the form 2^a 3^b 5^c 7^d (P:L130 FFT-friendly sizes;
- *                radices 2, 3, 5, 7 built), <= DGPE_MAX_N; nz even (the R2C half-spectrum, R#13).
+ *   nx, ny, nz   grid points per axis; each >= 4, of the form 2^a 3^b 5^c 7^d 11^e 13^f (P:L130 FFT-friendly
+ *                sizes), <= DGPE_MAX_N; nz even (the R2C half-spectrum, R#13).
  *   dx, dy, dz   grid spacings  (> 0);  dt  time step (> 0).
  *   gamma, nu, lambda   trap frequencies along x, y, z (R#2: gamma<->x slowest, lambda<->z).
  *   g, gdd       contact and dipolar interaction strengths; dipoles polarised along z (R#2).

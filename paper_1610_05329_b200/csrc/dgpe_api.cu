@@ -132,23 +132,23 @@ static int upload(dgpe_handle* h, const std::vector<T>& v, T** out)
     return DGPE_OK;
 }
 
-// FFT-friendly sizes built so far: 2^a 3^b 5^c 7^d (P:L130 also lists 11 and 13)
+// FFT-friendly sizes: 2^a 3^b 5^c 7^d 11^e 13^f
 static bool smooth2357(int n)
 {
     if (n < 1) return false;
-    for (int f : {2, 3, 5, 7})
+    for (int f : {2, 3, 5, 7, 11, 13})
         while (n % f == 0) n /= f;
     return n == 1;
 }
 
-// radices 8, 4, 2 first, then 3, 5, 7; butterfly slots per column = n / largest radix
+// radices 8, 4, 2 first, then 3, 5, 7, 11, 13; butterfly slots per column = n / largest radix
 static int make_plan(dgpe_handle* h, int n, FftPlan* P, cplx** tw_dev, int max_slots)
 {
     std::memset(P, 0, sizeof(*P));
     P->n = n;
     int m = n, np = 0, rmax = 1;
-    const int order[6] = {8, 4, 2, 3, 5, 7};
-    for (int oi = 0; oi < 6; ++oi) {
+    const int order[8] = {8, 4, 2, 3, 5, 7, 11, 13};
+    for (int oi = 0; oi < 8; ++oi) {
         const int R = order[oi];
         while (m % R == 0 && m > 1) {
             if (np >= MAX_PASSES) return fail(DGPE_ERR_UNSUPPORTED, "FFT length %d needs too many passes", n);
@@ -157,12 +157,15 @@ static int make_plan(dgpe_handle* h, int n, FftPlan* P, cplx** tw_dev, int max_s
             if (R > rmax) rmax = R;
         }
     }
-    if (m != 1) return fail(DGPE_ERR_ARG, "FFT length %d is not of the form 2^a 3^b 5^c 7^d", n);
+    if (m != 1) return fail(DGPE_ERR_ARG, "FFT length %d is not of the form 2^a 3^b 5^c 7^d 11^e 13^f", n);
     if (np == 0) {           // n == 1: one radix-1 "pass" does not exist; callers never ask for it
         return fail(DGPE_ERR_ARG, "FFT length %d too small", n);
     }
     P->npass = np;
-    P->nbf = std::min(n / rmax, max_slots);      // 8 * nbf threads per tile, bounded by the kernel (then a slot runs several butterflies)
+    // butterfly slots per line: n / (largest radix, at most 8) -- a slot then runs at most ceil(8/R) butterflies
+    // of a radix-R pass (radices 11 and 13 leave some slots idle) -- bounded by the kernel's thread limit
+    const int rdiv = std::min(rmax, 8);
+    P->nbf = std::min((n + rdiv - 1) / rdiv, max_slots);
     for (int p = 0; p < np; ++p) {
         const int nbut = n / P->radix[p];
         P->nb[p] = (nbut + P->nbf - 1) / P->nbf;
@@ -440,7 +443,7 @@ extern "C" dgpe_handle* dgpe_create(int nx, int ny, int nz, double dx, double dy
     const int ns[3] = {nx, ny, nz};
     for (int a = 0; a < 3; ++a) {
         if (ns[a] < 4) { fail(DGPE_ERR_ARG, "grid size %d < 4", ns[a]); return nullptr; }
-        if (!smooth2357(ns[a])) { fail(DGPE_ERR_ARG, "grid size %d is not of the form 2^a 3^b 5^c 7^d", ns[a]); return nullptr; }
+        if (!smooth2357(ns[a])) { fail(DGPE_ERR_ARG, "grid size %d is not of the form 2^a 3^b 5^c 7^d 11^e 13^f", ns[a]); return nullptr; }
         if (ns[a] > DGPE_MAX_N) { fail(DGPE_ERR_UNSUPPORTED, "grid size %d > %d", ns[a], DGPE_MAX_N); return nullptr; }
     }
     if (nz % 2) { fail(DGPE_ERR_ARG, "nz = %d must be even", nz); return nullptr; }

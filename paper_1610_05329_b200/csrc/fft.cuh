@@ -1,4 +1,4 @@
-// fft.cuh -- mixed-radix (2, 3, 4, 5, 7, 8) Stockham autosort FFT passes over a shared-memory tile of
+// fft.cuh -- mixed-radix (2, 3, 4, 5, 7, 8, 11, 13) Stockham autosort FFT passes over a shared-memory tile of
 // TILE_COLS lines (FFT-friendly sizes 2^a 3^b 5^c 7^d ...; BJ:north_star "mixed-radix (2^a 3^b)
 // shared-memory Stockham FFT passes per axis").
 //
@@ -52,7 +52,7 @@ struct Butterfly<3, INV> {
     }
 };
 
-// Odd prime radix R = 2h+1 (5, 7; P:L130 lists 2^a 3^b 5^c 7^d ... as the FFT-friendly sizes): with
+// Odd prime radix R = 2h+1 (5, 7, 11, 13: P:L130 lists 2^a 3^b 5^c 7^d 11^e 13^f as the FFT-friendly sizes): with
 // a_k = v_k + v_{R-k}, b_k = v_k - v_{R-k}  (k = 1..h)
 //   out_s, out_{R-s} = (v_0 + sum_k cos(2 pi s k/R) a_k)  -/+  i sum_k sin(2 pi s k/R) b_k   (forward; signs swap for the inverse)
 template <int R, bool INV>
@@ -114,6 +114,28 @@ struct Butterfly<7, INV> {
                              0.43388373911755812047576833284836, -0.43388373911755812047576833284836,
                              -0.97492791218182360701813168299393, -0.78183148246802980870844452667406};
         OddPrimeButterfly<7, INV>::run(v, C, S);
+    }
+};
+
+template <bool INV>
+struct Butterfly<11, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[11])
+    {
+        // cos, sin of 2 pi m/11
+        const double C[11] = {1.0, 0.8412535328311812, 0.41541501300188644, -0.142314838273285, -0.654860733945285, -0.9594929736144974, -0.9594929736144975, -0.6548607339452852, -0.14231483827328523, 0.41541501300188605, 0.8412535328311812};
+        const double S[11] = {0.0, 0.5406408174555976, 0.9096319953545183, 0.9898214418809328, 0.7557495743542583, 0.28173255684142967, -0.2817325568414294, -0.7557495743542582, -0.9898214418809327, -0.9096319953545186, -0.5406408174555974};
+        OddPrimeButterfly<11, INV>::run(v, C, S);
+    }
+};
+
+template <bool INV>
+struct Butterfly<13, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[13])
+    {
+        // cos, sin of 2 pi m/13
+        const double C[13] = {1.0, 0.8854560256532099, 0.5680647467311559, 0.120536680255323, -0.35460488704253545, -0.7485107481711012, -0.970941817426052, -0.9709418174260521, -0.7485107481711013, -0.3546048870425359, 0.1205366802553232, 0.5680647467311548, 0.88545602565321};
+        const double S[13] = {0.0, 0.4647231720437685, 0.8229838658936564, 0.992708874098054, 0.9350162426854148, 0.6631226582407952, 0.23931566428755768, -0.23931566428755743, -0.663122658240795, -0.9350162426854147, -0.992708874098054, -0.822983865893657, -0.4647231720437684};
+        OddPrimeButterfly<13, INV>::run(v, C, S);
     }
 };
 
@@ -235,6 +257,10 @@ __device__ __forceinline__ void fft_run(const FftPlan& P, int b, bool active,
             DGPE_PASS(5, 2)
             DGPE_PASS(7, 1)
             DGPE_PASS(7, 2)
+            DGPE_PASS(11, 1)
+            DGPE_PASS(11, 2)
+            DGPE_PASS(13, 1)
+            DGPE_PASS(13, 2)
             default: break;
         }
 #undef DGPE_PASS

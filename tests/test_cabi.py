@@ -35,11 +35,11 @@ def test_header_cites_the_paper_for_each_stage():
 
 
 @pytest.mark.parametrize("args,frag", [
-    ((64, 64, 66, .1, .1, .1, .01, 1, 1, 1, 1, 1, 0), "2^a 3^b 5^c 7^d"),       # 66 = 2*3*11
+    ((64, 64, 34, .1, .1, .1, .01, 1, 1, 1, 1, 1, 0), "2^a 3^b 5^c 7^d 11^e 13^f"),       # 34 = 2*17
     ((64, 64, 54, .1, .1, .1, .01, 1, 1, 1, 1, 1, 2), "mode"),
     ((2, 64, 64, .1, .1, .1, .01, 1, 1, 1, 1, 1, 0), "< 4"),
     ((64, 64, 27, .1, .1, .1, .01, 1, 1, 1, 1, 1, 0), "even"),
-    ((64, 52, 64, .1, .1, .1, .01, 1, 1, 1, 1, 1, 0), "2^a 3^b 5^c 7^d"),       # 52 = 4*13 (radices 11, 13 not built)
+    ((64, 76, 64, .1, .1, .1, .01, 1, 1, 1, 1, 1, 0), "2^a 3^b 5^c 7^d 11^e 13^f"),       # 76 = 4*19
     ((64, 64, 64, .1, -.1, .1, .01, 1, 1, 1, 1, 1, 0), "positive"),
     ((64, 64, 64, .1, .1, .1, 0.0, 1, 1, 1, 1, 1, 0), "positive"),
     ((2048, 64, 64, .1, .1, .1, .01, 1, 1, 1, 1, 1, 0), "> 1024"),

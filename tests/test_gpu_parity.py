@@ -102,7 +102,7 @@ def _smooth_lengths(lo=4, hi=1024):
     out = []
     for n in range(lo, hi + 1):
         m = n
-        for f in (2, 3, 5, 7):
+        for f in (2, 3, 5, 7, 11, 13):
             while m % f == 0:
                 m //= f
         if m == 1:
@@ -113,7 +113,7 @@ def _smooth_lengths(lo=4, hi=1024):
 @pytest.mark.parametrize("mode", [0, 1])
 @pytest.mark.parametrize("axis", [0, 1, 2])
 def test_every_supported_length_on_every_axis(gpu, oracle, axis, mode):
-    """One full step (imaginary or real time) for EVERY length 2^a 3^b 5^c 7^d in [4, 1024] on each axis (thin box in
+    """One full step (imaginary or real time) for EVERY length 2^a 3^b 5^c 7^d 11^e 13^f in [4, 1024] on each axis (thin box in
     the other two), against the oracle: every plan, specialised or generic, launches and is right."""
     worst = 0.0
     for n in _smooth_lengths():

@@ -51,7 +51,7 @@ def rand_c(shape, seed):
 
 @pytest.mark.parametrize("shape", [(8, 8, 8), (4, 8, 16),            # P1: radix 2 (BJ:north_star check 1)
                                    (6, 6, 6), (12, 6, 3), (9, 4, 6),  # P2: radix 3 and mixed
-                                   (5, 7, 10)])                       # generic odd primes fall through
+                                   (5, 7, 10), (11, 13, 22)])         # the other primes of P:L130
 @pytest.mark.parametrize("sign", [-1, 1])
 def test_p1_p2_dft3_is_brute_force_dft(oracle, shape, sign):
     a = rand_c(shape, 7)
@@ -60,7 +60,7 @@ def test_p1_p2_dft3_is_brute_force_dft(oracle, shape, sign):
     assert np.max(np.abs(got - ref)) <= 1e-12 * np.max(np.abs(ref))
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 4, 6, 8, 9, 12, 27, 64, 96, 384, 768])
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 6, 8, 9, 12, 27, 64, 96, 384, 768, 480, 500, 250, 143, 572, 1001])
 def test_p1_dft1_sizes(oracle, n):
     a = rand_c((n,), n)
     j = np.arange(n)
