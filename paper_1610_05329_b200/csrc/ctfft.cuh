@@ -45,16 +45,6 @@ __host__ __device__ constexpr int rmax(int n)
     while (n > 1) { int q = pick(n); if (q > r) r = q; n /= q; }
     return r;
 }
-__host__ __device__ constexpr bool smooth(int n)
-{
-    if (n < 1) return false;
-    while (n % 2 == 0) n /= 2;
-    while (n % 3 == 0) n /= 3;
-    while (n % 5 == 0) n /= 5;
-    while (n % 7 == 0) n /= 7;
-    return n == 1;
-}
-
 }  // namespace ct
 
 // Pass P of an N-point transform for a team of NBF butterfly slots (slot b handles butterflies
@@ -223,15 +213,5 @@ __device__ __forceinline__ void st_stream(cplx* p, cplx v)
 // L2 prefetch of the 128-byte line holding p: kernels ask for the data of the tile / line that will be
 // processed one "residency" later, so that the demand loads of that later CTA hit L2 instead of HBM
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); }
-
-// ---- cp.async (LDGSTS): 16 bytes per thread straight into shared memory, L2-only caching ----
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
-{
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int NKEEP>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(NKEEP) : "memory"); }
 
 }  // namespace dgpe

@@ -856,7 +856,6 @@ static bool tma_sweep_ok(const dgpe_handle* h, const LineMap& m, const AxisSweep
     // three stages when only one CTA fits on an SM anyway (tiles of 64 KB); two stages and several CTAs
     // per SM for the short lines, whose CTAs are small
     *nstage = (ns >= 3 && tile > 40 * 1024) ? 3 : 2;
-    if (const char* e = getenv("DGPE_TMA_STAGES")) { const int v = atoi(e); if (v >= 2 && v <= ns && v <= 3) *nstage = v; }
     *box_rows = m.n / nbox;
     return true;
 }
