@@ -21,14 +21,25 @@ __host__ __device__ constexpr int pick(int m)
 {
     return (m % 8 == 0) ? 8 : (m % 4 == 0) ? 4 : (m % 2 == 0) ? 2 : (m % 3 == 0) ? 3 : (m % 5 == 0) ? 5 : 7;
 }
+// Lengths whose plan starts with a radix other than pick()'s: n/32 for the z-line transforms of nz = 192,
+// 320, 384 (M = 96, 160, 192), so that their first pass is one butterfly per lane, fed from registers
+// with every lane busy (zline.cuh).  Any radix order is a valid transform; the x/y kernels of the same
+// lengths simply use the same plan.
+__host__ __device__ constexpr int first_of(int n) { return n == 192 ? 6 : n == 160 ? 5 : n == 96 ? 3 : 0; }
 __host__ __device__ constexpr int npass(int n)
 {
     int c = 0;
+    if (first_of(n)) { n /= first_of(n); ++c; }
     while (n > 1) { n /= pick(n); ++c; }
     return c;
 }
 __host__ __device__ constexpr int radix_fwd(int n, int p)
 {
+    if (first_of(n)) {
+        if (p == 0) return first_of(n);
+        n /= first_of(n);
+        --p;
+    }
     for (int i = 0; i < p; ++i) n /= pick(n);
     return pick(n);
 }
@@ -42,6 +53,7 @@ __host__ __device__ constexpr int ns_at(int n, int p, bool rev)
 __host__ __device__ constexpr int rmax(int n)
 {
     int r = 1;
+    if (first_of(n)) { r = first_of(n); n /= r; }
     while (n > 1) { int q = pick(n); if (q > r) r = q; n /= q; }
     return r;
 }

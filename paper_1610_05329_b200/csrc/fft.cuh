@@ -152,6 +152,28 @@ struct Butterfly<4, INV> {
     }
 };
 
+// 6 = 2 x 3: two radix-3 butterflies on the even and the odd inputs, twiddles w_6^k, one radix-2 step
+template <bool INV>
+struct Butterfly<6, INV> {
+    static __device__ __forceinline__ void run(cplx (&v)[6])
+    {
+        const double S = 0.86602540378443864676372317075294;   // sin(pi/3)
+        cplx e[3] = {v[0], v[2], v[4]};
+        cplx o[3] = {v[1], v[3], v[5]};
+        Butterfly<3, INV>::run(e);
+        Butterfly<3, INV>::run(o);
+        // w_6 = 1/2 -/+ i S (forward / inverse), w_6^2 = -1/2 -/+ i S
+        const cplx w1 = INV ? mk(0.5, S) : mk(0.5, -S), w2 = INV ? mk(-0.5, S) : mk(-0.5, -S);
+        const cplx o1 = cmul(o[1], w1), o2 = cmul(o[2], w2);
+        v[0] = cadd(e[0], o[0]);
+        v[3] = csub(e[0], o[0]);
+        v[1] = cadd(e[1], o1);
+        v[4] = csub(e[1], o1);
+        v[2] = cadd(e[2], o2);
+        v[5] = csub(e[2], o2);
+    }
+};
+
 template <bool INV>
 struct Butterfly<8, INV> {
     static __device__ __forceinline__ void run(cplx (&v)[8])
