@@ -380,3 +380,66 @@ def test_fullsize_step_properties(gpu, c4):
     mu = G0.chempot(p1)
     assert abs(mu - 0.5 * sum(cfg.trap)) <= 0.5 * sum(w * w * d * d / 16 for w, d in zip(cfg.trap, cfg.d)) + 5e-3
     assert abs(mu - G0.energy(p1)) <= 1e-12        # no interaction: mu == E
+
+
+# ------------------------------------------------------------------------------------------------
+# BJ:configs[4] at its full size (768 x 768 x 384, real time): the 768- and 384-point kernels in the
+# launch configuration bench.py --config C5 times
+# ------------------------------------------------------------------------------------------------
+
+def test_fullsize_c5_sweeps_dipolar_and_norm(gpu, oracle):
+    cfg = inputs.CONFIGS["C5"]
+    nx, ny, nz = cfg.shape
+    G = gpu.Dgpe(*cfg.create_args())
+    gen = torch.Generator(device="cuda").manual_seed(31)
+    psi = torch.randn(cfg.shape, dtype=torch.float64, device="cuda", generator=gen).to(torch.complex128)
+    psi += 1j * torch.randn(cfg.shape, dtype=torch.float64, device="cuda", generator=gen)
+    rng = np.random.default_rng(32)
+    # (c) each sweep on 64 sampled lines per axis (edge lines included) against the oracle's solve
+    for axis in range(3):
+        n = cfg.shape[axis]
+        na, nb = [cfg.shape[a] for a in range(3) if a != axis]
+        out = psi.clone()
+        G.sweep(out, axis)
+        ia, ib = rng.integers(0, na, 64), rng.integers(0, nb, 64)
+        ia[:4], ib[:4] = [0, 0, na - 1, na - 1], [0, nb - 1, 0, nb - 1]
+        sel = (torch.from_numpy(ia).cuda(), torch.from_numpy(ib).cuda())
+        if axis == 0:
+            lin, lout = psi[:, sel[0], sel[1]], out[:, sel[0], sel[1]]
+        elif axis == 1:
+            lin, lout = psi[sel[0], :, sel[1]].T, out[sel[0], :, sel[1]].T
+        else:
+            lin, lout = psi[sel[0], sel[1], :].T, out[sel[0], sel[1], :].T
+        O = oracle.Oracle(n, 8, 8, cfg.d[axis], 1.0, 1.0, cfg.dt, 1, 1, 1, 0.0, 0.0, cfg.mode)
+        a = np.ascontiguousarray(lin.cpu().numpy().reshape(n, 8, 8))
+        O.sweep(a, 0)
+        assert np.max(np.abs(lout.cpu().numpy().reshape(n, 8, 8) - a)) <= TOL_1, axis
+        del out
+    del psi
+    torch.cuda.empty_cache()
+    # (a) Phi of plane-wave densities against the closed form (pin P4) through K1-K5
+    L = [n * d for n, d in zip(cfg.shape, cfg.d)]
+    x, y, z = [torch.from_numpy(inputs.coords(n, d)).cuda() for n, d in zip(cfg.shape, cfg.d)]
+    dens = torch.ones(cfg.shape, dtype=torch.float64, device="cuda")
+    phi_ref = torch.zeros_like(dens)
+    for m, amp, ph in [((3, 0, 0), 0.11, 0.3), ((0, 0, 5), 0.07, 1.1), ((2, -7, 1), 0.05, 2.0), ((-300, 31, 191), 0.02, 0.5),
+                       ((0, 384, 0), 0.01, 0.0)]:
+        q = [2 * np.pi * mi / Li for mi, Li in zip(m, L)]
+        udd = (4 * np.pi / 3) * (3 * q[2] ** 2 / (q[0] ** 2 + q[1] ** 2 + q[2] ** 2) - 1)
+        w = torch.cos(q[0] * x[:, None, None] + q[1] * y[None, :, None] + q[2] * z[None, None, :] + ph)
+        dens += amp * w
+        phi_ref += udd * amp * w
+        del w
+    psi = torch.sqrt(dens).to(torch.complex128)
+    del dens
+    phi = G.dipolar(psi)
+    assert float((phi - phi_ref).abs().max()) <= 1e-12
+    del phi, phi_ref, psi
+    torch.cuda.empty_cache()
+    # the literal config: real time conserves the norm (BJ:north_star check 4) over 10 steps of the seeded state
+    psi = dev(inputs.initial_state(cfg))
+    n0 = G.norm(psi)
+    assert G.step(psi, 10) == gpu.OK
+    assert abs(G.norm(psi) - n0) <= 1e-12
+    for face in (psi[0], psi[-1], psi[:, 0], psi[:, -1], psi[:, :, 0], psi[:, :, -1]):
+        assert float(face.abs().max()) == 0.0
