@@ -657,7 +657,7 @@ static int launch_fft_xy_n(dgpe_handle* h, const LineMap& map, int nbatch, const
     int ctas_per_sm = 0;
     int rc = kernel_setup((const void*)kern, xy_threads<N>(), smem, &ctas_per_sm);
     if (rc) return rc;
-    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 1.0 / (double)h->N,
+    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 2.0 * 3.14159265358979323846264338327950288 / ((double)h->nx * h->dx), 1.0 / (double)h->N,
               (h->prefetch & (KIND == FFT_X_UDD ? PF_FFT_X : PF_FFT_Y)) ? h->pf_mult * ctas_per_sm * h->num_sms : 0};
     dim3 grid((map.ncols + TILE_COLS - 1) / TILE_COLS, nbatch);
     kern<<<grid, xy_threads<N>(), smem, h->stream>>>(h->spec, map, tw, U);

@@ -22,6 +22,7 @@ namespace dgpe {
 struct UddArgs {
     int nzh;                          // kz bins per row of the half-spectrum
     const double *kx2, *ky2, *kz2;    // squared wave numbers (R#10, R#11)
+    double dkx;                       // 2 pi/(nx dx): kx of bin m is (m <= nx/2 ? m : m - nx) dkx
     double invN;                      // 1/(nx ny nz): normalisation of the inverse transform (R#10)
     int pf_tiles;                     // L2 prefetch distance in tiles (one residency of CTAs); 0 = off
 };
@@ -79,6 +80,10 @@ k_fft_xy(cplx* __restrict__ data, LineMap map, const cplx* __restrict__ tw, UddA
     if constexpr (KIND != FFT_X_UDD) {
         ct_fft_range<N, KIND == FFT_INV, false, NBF, SyncCta, PosTile, 0, L, true>(colsm, b, on, tw, from_g, to_g);
     } else {
+        // ky^2, kz^2 of this thread's column, loaded now and used after the forward passes
+        const int ky = (colok ? col : 0) / U.nzh, kz = (colok ? col : 0) - ky * U.nzh;
+        const double qy = __ldg(&U.ky2[ky]), qz = __ldg(&U.kz2[kz]);
+        const bool origin_col = (ky == 0 && kz == 0);
         // forward passes 0 .. L-2 through the tile
         ct_fft_range<N, false, false, NBF, SyncCta, PosTile, 0, L - 1, true>(colsm, b, on, tw, from_g, to_g);
         // last forward pass, Udd~(k)/N, first inverse pass: one set of registers
@@ -96,12 +101,12 @@ k_fft_xy(cplx* __restrict__ data, LineMap map, const cplx* __restrict__ tw, UddA
         if (on) {
             pf.bfly(b);
             // Udd~(k) = (4 pi/3)(3 kz^2/|k|^2 - 1), Udd~(0) = 0 (BJ:configs[0]; R#11); column = (ky, kz) flattened
-            const int ky = col / U.nzh, kz = col - ky * U.nzh;
-            const double qy = __ldg(&U.ky2[ky]), qz = __ldg(&U.kz2[kz]);
             const double FOUR_PI_3 = 4.1887902047863909846168578443727;
-            const bool origin_col = (ky == 0 && kz == 0);
             pf.modify(b, [&](int idx, cplx v) {
-                const double k2 = __ldg(&U.kx2[idx]) + qy + qz;
+                // kx^2 from the bin index (f = idx or idx - N, R#10) instead of a table load whose latency
+                // would sit in the middle of the register chain
+                const double kx = (double)(idx <= N / 2 ? idx : idx - N) * U.dkx;
+                const double k2 = kx * kx + qy + qz;
                 // 1/k2 by two Newton steps from the single-precision reciprocal (<= 2 ulp; k2 is a sum of
                 // squared wave numbers, far inside the float range; k2 = 0 gives inf/NaN, replaced below)
                 double rk = (double)__frcp_rn((float)k2);
