@@ -15,6 +15,7 @@
 #pragma once
 #include "tma.cuh"
 #include "xysweep.cuh"
+#include <type_traits>
 
 namespace dgpe {
 
@@ -52,11 +53,24 @@ k_sweep_tma(const __grid_constant__ CUtensorMap tmap, TmaWalk W, SweepTables<CT>
     const int first = blockIdx.x, stride = gridDim.x;
     const int nmine = (first < W.ntiles) ? (W.ntiles - first + stride - 1) / stride : 0;
 
+    // Table entries.  With CONSTTAB only chunk 0 differs from the converged entries, and chunk 0 lives in warp 0:
+    // the other warps take the MIXED = false instantiation of each phase, whose table operands are plain
+    // constant-bank reads with no per-element select.
+    // (It pays with complex tables, real time: 768-point y sweep 1.64 -> 1.24 ms; with real tables the plain
+    // selects are as fast, so there every warp takes the MIXED path.)
     const bool g0 = g == 0;
-    auto t_inv = [&](int i) { if constexpr (CONSTTAB) return g0 ? P.inv0[i] : P.invU[i]; else return __ldg(&T.inv[s + i]); };
-    auto t_cc = [&](int i) { if constexpr (CONSTTAB) return g0 ? P.cc0[i] : P.ccU[i]; else return __ldg(&T.cc[s + i]); };
-    auto t_F = [&](int i) { if constexpr (CONSTTAB) return P.fU[i]; else return __ldg(&T.F[s + i]); };
-    auto t_Gm = [&](int i) { if constexpr (CONSTTAB) return g0 ? P.gm0[i] : P.gmU[i]; else return __ldg(&T.Gm[s + i]); };
+    using MixedT = std::true_type;
+    using PlainT = std::false_type;
+    constexpr bool SPLIT = CONSTTAB && sizeof(CT) != sizeof(double);
+    const bool warp0 = tid < 32;
+    auto run = [&](auto&& phase) {
+        if constexpr (SPLIT) { if (warp0) phase(MixedT{}); else phase(PlainT{}); }
+        else phase(MixedT{});
+    };
+    auto t_inv = [&](auto M, int i) { if constexpr (!CONSTTAB) return __ldg(&T.inv[s + i]); else if constexpr (decltype(M)::value) return g0 ? P.inv0[i] : P.invU[i]; else return P.invU[i]; };
+    auto t_cc = [&](auto M, int i) { if constexpr (!CONSTTAB) return __ldg(&T.cc[s + i]); else if constexpr (decltype(M)::value) return g0 ? P.cc0[i] : P.ccU[i]; else return P.ccU[i]; };
+    auto t_F = [&](auto M, int i) { if constexpr (!CONSTTAB) return __ldg(&T.F[s + i]); else return P.fU[i]; };
+    auto t_Gm = [&](auto M, int i) { if constexpr (!CONSTTAB) return __ldg(&T.Gm[s + i]); else if constexpr (decltype(M)::value) return g0 ? P.gm0[i] : P.gmU[i]; else return P.gmU[i]; };
 
     auto coords = [&](int it, int& c0, int& c2) {
         const int t = first + it * stride;
@@ -99,16 +113,19 @@ k_sweep_tma(const __grid_constant__ CUtensorMap tmap, TmaWalk W, SweepTables<CT>
         // ---- A: local forward elimination with zero inflow ----
         cplx ev[LC];
         cplx e = mk(0.0, 0.0);
+        auto phaseA = [&](auto M) {
 #pragma unroll
-        for (int i = 0; i < LC; ++i) {
-            ev[i] = mk(0.0, 0.0);
-            if (work && i < cnt) {
-                cplx d = coef_mul(T.r, cadd(p[i], p[i + 2]));
-                d = coef_fma(T.omr2, p[i + 1], d);
-                e = coef_fma(coef_neg(t_cc(i)), e, coef_mul(t_inv(i), d));
-                ev[i] = e;
+            for (int i = 0; i < LC; ++i) {
+                ev[i] = mk(0.0, 0.0);
+                if (work && i < cnt) {
+                    cplx d = coef_mul(T.r, cadd(p[i], p[i + 2]));
+                    d = coef_fma(T.omr2, p[i + 1], d);
+                    e = coef_fma(coef_neg(t_cc(M, i)), e, coef_mul(t_inv(M, i), d));
+                    ev[i] = e;
+                }
             }
-        }
+        };
+        run(phaseA);
         if (work) smE[g][c] = e;
         __syncthreads();                                 // every thread has read its part of the tile
 
@@ -124,14 +141,17 @@ k_sweep_tma(const __grid_constant__ CUtensorMap tmap, TmaWalk W, SweepTables<CT>
         if (work) {
             cplx ein = mk(0.0, 0.0);
             for (int h = max(0, g - T.Kf); h < g; ++h) ein = coef_fma(__ldg(&T.Ach[h]), ein, smE[h][c]);
+            auto phaseC = [&](auto M) {
 #pragma unroll
-            for (int i = LC - 1; i >= 0; --i) {
-                if (i < cnt) {
-                    const cplx ee = coef_fma(t_F(i), ein, ev[i]);
-                    x = coef_fma(coef_neg(t_cc(i)), x, ee);
-                    ev[i] = x;
+                for (int i = LC - 1; i >= 0; --i) {
+                    if (i < cnt) {
+                        const cplx ee = coef_fma(t_F(M, i), ein, ev[i]);
+                        x = coef_fma(coef_neg(t_cc(M, i)), x, ee);
+                        ev[i] = x;
+                    }
                 }
-            }
+            };
+            run(phaseC);
             smX[g][c] = x;
         }
         __syncthreads();
@@ -142,14 +162,17 @@ k_sweep_tma(const __grid_constant__ CUtensorMap tmap, TmaWalk W, SweepTables<CT>
             for (int h = min(T.G - 1, g + T.Kb); h > g; --h) xin = coef_fma(__ldg(&T.Bch[h]), xin, smX[h][c]);
             if (g == 0) col[0] = mk(0.0, 0.0);
             if (t_end == n - 1) col[(n - 1) * TILE_COLS] = mk(0.0, 0.0);
+            auto phaseE = [&](auto M) {
 #pragma unroll
-            for (int i = 0; i < LC; ++i) {
-                if (i < cnt) {
-                    const cplx v = coef_fma(t_Gm(i), xin, ev[i]);
-                    nrm += cabs2(v);
-                    col[(s + i) * TILE_COLS] = v;
+                for (int i = 0; i < LC; ++i) {
+                    if (i < cnt) {
+                        const cplx v = coef_fma(t_Gm(M, i), xin, ev[i]);
+                        nrm += cabs2(v);
+                        col[(s + i) * TILE_COLS] = v;
+                    }
                 }
-            }
+            };
+            run(phaseE);
         }
         fence_proxy_async();                             // my tile writes -> visible to the TMA store
         __syncthreads();
