@@ -1,0 +1,34 @@
+"""bench.py contract checks that need no GPU: the reference arm (the oracle timed on the host cores) prints
+one JSON line with the keys the driver reads, and the roofline helpers read the committed profile data."""
+import json
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_reference_arm_prints_one_json_line():
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1", "--warmup", "0"],
+                         capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1
+    j = json.loads(lines[0])
+    assert j["impl"] == "reference" and j["metric"] == "sscn_steps_per_s" and j["unit"] == "steps/s"
+    assert j["higher_is_better"] is True and j["vs_baseline"] is None and j["dtype"] == "f64"
+    assert j["value"] > 0 and abs(j["ms_per_step"] * j["value"] - 1e3) < 1e-6 * 1e3
+    assert j["cpu_baseline"]["kind"] == "oracle" and j["cpu_baseline"]["cores"] == 1
+    assert j["e2e"] == {"value": j["value"], "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert "C4" in j["config"]["workload"] and "512x512x512" in j["config"]["workload"]
+
+
+def test_traffic_table_names_the_kernels_of_the_step():
+    sys.path.insert(0, ROOT)
+    import bench
+    for name in ("K1 dens_r2c(z)", "K3 fft_x*Udd*ifft_x", "K5+K8 c2r(z)+nonlinear+sweep_z", "K7 sweep_y(+norm)"):
+        t = bench.ncu_traffic(name)
+        assert t is not None and 1e9 < t < 1e10, name
+    assert bench.ncu_traffic("no such kernel") is None
+    peak, src = bench.load_peaks()
+    assert 3000 < peak < 9000 and ("measured" in src or "fallback" in src)
