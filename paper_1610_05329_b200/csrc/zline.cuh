@@ -4,17 +4,18 @@
 // "for the z sweep, the contiguous axis, tiles are ... staged in shared memory so the recursion runs
 // along a transposed tile").
 //
-// A z-line is contiguous in global memory, so a warp reads and writes it with fully coalesced 512-byte
-// accesses and needs no neighbouring lines: every line is an independent job of one warp, synchronised
-// with __syncwarp only.  Many warps per SM (16 at 512^3) are in different phases at any time, which
-// overlaps the loads, the shared-memory passes, the fp64 arithmetic and the stores without block
-// barriers.
+// A z-line is contiguous in global memory, so a warp reads and writes it with fully coalesced accesses
+// and needs no neighbouring lines: every line is an independent job of one warp (of one team of lanes
+// for nz <= 256), synchronised with __syncwarp only.  The launchers give every warp its own CTA, so a
+// finished line frees its slot at once; 16 (K5) to 28 (K1) warps per SM are in different phases at any
+// time, which overlaps the loads, the shared-memory passes, the fp64 arithmetic and the stores without
+// block barriers.
 //
 //   k_z_r2c   (K1)   n = s2 |psi|^2 -> packed nz/2-point FFT -> Hermitian split -> nz/2+1 bins
 //   k_z_main  (K5, K8, or both fused) Hermitian merge -> nz/2-point inverse FFT = Phi -> nonlinear
 //             exponential -> Crank-Nicolson sweep along z with the chunk of each lane in registers
 //
-// Shared memory per warp:
+// Shared memory per line:
 //   B  FFT buffer, M = nz/2 complex, element idx at idx + (idx >> 3)  (the one pad per 8 elements makes
 //      the stride-R writes of the first pass conflict free); the last inverse pass leaves Phi in it as
 //      nz plain doubles;
