@@ -29,12 +29,26 @@ def nvcc():
     raise RuntimeError("nvcc not found")
 
 
+STAMP = LIB + ".srchash"
+
+
+def source_hash():
+    """sha256 over the sources, the public header, this script and the flags: what libdgpe.so was built from.
+    (Not modification times: a copied tree -- gpurun, a fresh checkout -- keeps contents, not mtimes.)"""
+    import hashlib
+    h = hashlib.sha256()
+    for path in [os.path.join(CSRC, d) for d in sorted(DEPS)] + [HEADER, os.path.abspath(__file__)]:
+        with open(path, "rb") as f:
+            h.update(f.read())
+    h.update(" ".join(NVCC_FLAGS).encode())
+    return h.hexdigest()
+
+
 def up_to_date():
-    if not os.path.exists(LIB):
+    if not (os.path.exists(LIB) and os.path.exists(STAMP)):
         return False
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, d) for d in DEPS] + [HEADER, os.path.abspath(__file__)]
-    return all(os.path.getmtime(d) <= t for d in deps)
+    with open(STAMP) as f:
+        return f.read().strip() == source_hash()
 
 
 def build(force=False, verbose=False):
@@ -48,6 +62,8 @@ def build(force=False, verbose=False):
         sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
         raise RuntimeError("nvcc failed building libdgpe.so")
+    with open(STAMP, "w") as f:
+        f.write(source_hash() + "\n")
     return LIB
 
 
