@@ -38,17 +38,21 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C4")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--rpsi", action="store_true",
+                    help="imaginary-time configs: time the real-valued-psi path DGPE_IMAG_RPSI (SURVEY 8f NEXT-2); "
+                         "not the headline, which stays complex psi as BASELINE.json states")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
 
 
-def workload_name(cfg):
+def workload_name(cfg, rpsi=False):
     nx, ny, nz = cfg.shape
     mode = "imaginary-time" if cfg.mode == 0 else "real-time"
     src = (f"BASELINE.json configs[{int(cfg.name[1]) - 1}]" if cfg.name[0] == "C" else
            "grid of the paper's timing table " + cfg.name[1] + ", physics borrowed from C4: context only")
-    return (f"{cfg.name}: {mode} dipolar GPE {nx}x{ny}x{nz} fp64 complex, dx={cfg.d[0]} dt={cfg.dt} "
+    kind = "fp64 REAL-valued psi (DGPE_IMAG_RPSI, SURVEY 8f NEXT-2; same step, 8 bytes per point)" if rpsi else "fp64 complex"
+    return (f"{cfg.name}: {mode} dipolar GPE {nx}x{ny}x{nz} {kind}, dx={cfg.d[0]} dt={cfg.dt} "
             f"trap={cfg.trap} g={cfg.g} gdd={cfg.gdd} ({src})")
 
 
@@ -192,8 +196,16 @@ def run_b200(args, cfg):
     K, W = args.steps, max(args.warmup, 3)
     mycfg = replace(cfg, seed=replicas.replica_seed(cfg.seed, rank))       # each replica: its own seeded state
 
-    G = binding.Dgpe(*mycfg.create_args())
-    psi_host = torch.from_numpy(inputs.initial_state(mycfg)).pin_memory()
+    rpsi = bool(args.rpsi)
+    if rpsi and cfg.mode != 0:
+        raise SystemExit("--rpsi needs an imaginary-time config")
+    G = binding.Dgpe(*mycfg.create_args()[:-1], binding.IMAG_RPSI if rpsi else mycfg.mode)
+    state = inputs.initial_state(mycfg)
+    if rpsi:
+        import numpy as np
+        state = np.ascontiguousarray(state.real)          # the imaginary-time initial states are real
+    psi_host = torch.from_numpy(state).pin_memory()
+    del state
     psi0 = psi_host.cuda()
     psi = psi0.clone()
 
@@ -215,7 +227,7 @@ def run_b200(args, cfg):
     clocks = sampler.stop() if rank == 0 else None
     sec_local = e0.elapsed_time(e1) * 1e-3
     value, sec = replicas.aggregate_throughput(K, sec_local)
-    finite = bool(torch.isfinite(torch.view_as_real(psi)).all())
+    finite = bool(torch.isfinite(psi if rpsi else torch.view_as_real(psi)).all())
 
     # ---- per-kernel durations, CUDA events on the handle's stream (dgpe_step_profile) ----
     psi.copy_(psi0)
@@ -233,7 +245,8 @@ def run_b200(args, cfg):
     step_gbps = G.bytes_per_step / step_ms * 1e-6
     built = sum(k["bytes"] for k in kernels)
     whole = {"algorithmic_bytes_per_step": G.bytes_per_step, "achieved": step_gbps, "frac": step_gbps / peak,
-             "unit": "GB/s", "model": "M1 = 144N + 8S (SURVEY section 8d; DESIGN.md section 7)",
+             "unit": "GB/s", "model": ("M1r = 72N + 8S (real-valued psi: SURVEY section 8f NEXT-2; DESIGN.md section 7)" if rpsi
+                                        else "M1 = 144N + 8S (SURVEY section 8d; DESIGN.md section 7)"),
              "frac_of_nominal_8TBps": step_gbps / 8000.0,
              "as_built": {"bytes_per_step": built, "achieved": built / step_ms * 1e-6,
                           "frac": built / step_ms * 1e-6 / peak,
@@ -253,7 +266,7 @@ def run_b200(args, cfg):
         e2e_local = time.perf_counter() - t0
         replicas.barrier()
         e2e_value, _ = replicas.aggregate_throughput(K, e2e_local)
-        nbytes = work.numel() * 16
+        nbytes = work.numel() * work.element_size()
         e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes / K, "d2h_bytes_per_step": nbytes / K,
                "call": f"dgpe_step_host(psi_pinned, {K}): one H2D of psi ({nbytes} B), {K} steps, one D2H; bytes per "
                        f"step = bytes per call / {K}", "ms_per_call": e2e_local * 1e3}
@@ -267,9 +280,9 @@ def run_b200(args, cfg):
         "ms_per_step": sec / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "grid_pt_updates_per_s": value * cfg.npoints,
-        "config": {"workload": workload_name(cfg), "parallelism": f"replicas x{world} (no sharding, no collectives)",
+        "config": {"workload": workload_name(cfg, rpsi), "parallelism": f"replicas x{world} (no sharding, no collectives)",
                    "l2": "inputs larger than L2: psi %.2f GB + half-spectrum %.2f GB vs 126 MB" %
-                         (cfg.npoints * 16e-9, cfg.shape[0] * cfg.shape[1] * (cfg.shape[2] // 2 + 1) * 16e-9),
+                         (cfg.npoints * (8e-9 if rpsi else 16e-9), cfg.shape[0] * cfg.shape[1] * (cfg.shape[2] // 2 + 1) * 16e-9),
                    "status": int(status), "finite": finite,
                    "note": "literal C4 is in the dipolar-collapse regime: NaN from step ~19 (DESIGN.md section 4); "
                            "timing is data-independent"},

@@ -42,7 +42,19 @@ extern "C" {
 
 typedef struct dgpe_handle dgpe_handle;
 
-enum { DGPE_IMAG = 0, DGPE_REAL = 1 };
+/*
+ * DGPE_IMAG_RPSI -- imaginary time with a REAL-VALUED wave function (the
+ * paper's imaginary-time programs run ~1.65x faster than its real-time ones).  Every factor of the
+ * imaginary-time step is real (exp(-dt H), the Crank-Nicolson matrices with r = dt/(4 d^2), the norm), so a
+ * real psi stays real and the imaginary part of a complex psi carries nothing (R#5; the oracle's imaginary
+ * part stays exactly 0 for real input: tests/test_oracle_pins.py).  In this mode every `psi` argument is
+ * nx*ny*nz plain DOUBLES (8 bytes per point, same row-major layout, 16-byte aligned) and the step moves
+ * 72N + 8S bytes instead of 144N + 8S.  The results equal those of DGPE_IMAG on the same psi with a zero
+ * imaginary part.  nz must be one of the specialised z lengths (64, 128, 160, 192, 240, 250, 256, 320, 384,
+ * 480, 500, 512, 640, 768), else dgpe_create fails with DGPE_ERR_UNSUPPORTED.  The observables copy psi into
+ * a complex array the handle owns (16*nx*ny*nz bytes, allocated on first use).
+ */
+enum { DGPE_IMAG = 0, DGPE_REAL = 1, DGPE_IMAG_RPSI = 2 };
 
 enum {
     DGPE_OK = 0,
@@ -60,7 +72,7 @@ enum {
  *   dx, dy, dz   grid spacings  (> 0);  dt  time step (> 0).
  *   gamma, nu, lambda   trap frequencies along x, y, z (R#2: gamma<->x slowest, lambda<->z).
  *   g, gdd       contact and dipolar interaction strengths; dipoles polarised along z (R#2).
- *   mode         DGPE_IMAG or DGPE_REAL.
+ *   mode         DGPE_IMAG, DGPE_REAL or DGPE_IMAG_RPSI.
  * Returns NULL on error (DGPE_ERR_ARG / UNSUPPORTED / NOMEM / CUDA in dgpe_last_error()).
  * Uses the current CUDA device; allocates 16*nx*ny*(nz/2+1) bytes plus O(nx+ny+nz) tables.
  */

@@ -10,7 +10,7 @@ import torch
 
 from . import build as _build
 
-IMAG, REAL = 0, 1
+IMAG, REAL, IMAG_RPSI = 0, 1, 2
 OK, ERR_ARG, ERR_CUDA, ERR_NOMEM, ERR_UNSUPPORTED, ERR_NONFINITE = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ("dgpe_create", "dgpe_destroy", "dgpe_set_stream", "dgpe_step", "dgpe_norm", "dgpe_chempot",
@@ -71,13 +71,15 @@ def _check(rc):
 
 
 class Dgpe:
-    """One dgpe_handle.  psi arguments are contiguous torch.complex128 CUDA tensors of shape (nx, ny, nz)."""
+    """One dgpe_handle.  psi arguments are contiguous torch.complex128 CUDA tensors of shape (nx, ny, nz)
+    (torch.float64 for mode IMAG_RPSI, the real-valued imaginary-time path)."""
 
     def __init__(self, nx, ny, nz, dx, dy, dz, dt, gamma, nu, lam, g, gdd, mode, stream=None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1610_05329_b200 needs a CUDA device (no CPU fallback)")
         self.shape = (nx, ny, nz)
         self.mode = mode
+        self.dtype = torch.float64 if mode == IMAG_RPSI else torch.complex128
         self.h = lib().dgpe_create(nx, ny, nz, dx, dy, dz, dt, gamma, nu, lam, g, gdd, mode)
         if not self.h:
             raise DgpeError(ERR_ARG, last_error())
@@ -99,9 +101,9 @@ class Dgpe:
         _check(lib().dgpe_set_stream(self.h, C.c_void_p(ptr)))
 
     def _psi(self, psi):
-        if not (isinstance(psi, torch.Tensor) and psi.is_cuda and psi.dtype == torch.complex128
+        if not (isinstance(psi, torch.Tensor) and psi.is_cuda and psi.dtype == self.dtype
                 and psi.is_contiguous() and tuple(psi.shape) == self.shape):
-            raise TypeError(f"psi must be a contiguous CUDA complex128 tensor of shape {self.shape}")
+            raise TypeError(f"psi must be a contiguous CUDA {self.dtype} tensor of shape {self.shape}")
         return C.c_void_p(psi.data_ptr())
 
     def step(self, psi, nsteps=1):
@@ -112,10 +114,10 @@ class Dgpe:
         return rc
 
     def step_host(self, psi_host, nsteps=1):
-        """dgpe_step_host on a contiguous CPU complex128 tensor (pinned for full-speed copies)."""
-        if not (isinstance(psi_host, torch.Tensor) and not psi_host.is_cuda and psi_host.dtype == torch.complex128
+        """dgpe_step_host on a contiguous CPU tensor of the handle's dtype (pinned for full-speed copies)."""
+        if not (isinstance(psi_host, torch.Tensor) and not psi_host.is_cuda and psi_host.dtype == self.dtype
                 and psi_host.is_contiguous() and tuple(psi_host.shape) == self.shape):
-            raise TypeError(f"psi_host must be a contiguous CPU complex128 tensor of shape {self.shape}")
+            raise TypeError(f"psi_host must be a contiguous CPU {self.dtype} tensor of shape {self.shape}")
         rc = lib().dgpe_step_host(self.h, C.c_void_p(psi_host.data_ptr()), int(nsteps))
         if rc not in (OK, ERR_NONFINITE):
             _check(rc)

@@ -19,6 +19,7 @@ NVCC_FLAGS = [
     "-O3", "-std=c++17", "-lineinfo",
     "-shared", "-Xcompiler", "-fPIC",
     "-cudart", "static",
+    "-split-compile", "0",      # optimise the kernels of the one translation unit on all host cores
 ]
 
 

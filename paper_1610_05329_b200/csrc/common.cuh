@@ -34,6 +34,15 @@ __device__ __forceinline__ cplx coef_fma(cplx c, cplx b, cplx a)
     return mk(fma(c.x, b.x, fma(-c.y, b.y, a.x)), fma(c.x, b.y, fma(c.y, b.x, a.y)));
 }
 
+// Real-valued psi (imaginary time, SV section 8f NEXT-2): the same sweep arithmetic on plain doubles.
+__device__ __forceinline__ double cadd(double a, double b) { return a + b; }
+__device__ __forceinline__ double cabs2(double a) { return a * a; }
+__device__ __forceinline__ double coef_mul(double c, double v) { return c * v; }
+__device__ __forceinline__ double coef_fma(double c, double b, double a) { return fma(c, b, a); }
+// p ? a : b, per component
+__device__ __forceinline__ double el_sel(bool p, double a, double b) { return p ? a : b; }
+__device__ __forceinline__ cplx el_sel(bool p, cplx a, cplx b) { return mk(p ? a.x : b.x, p ? a.y : b.y); }
+
 // Mixed-radix plan of one 1-D transform length (built on the host in dgpe_api.cu).
 struct FftPlan {
     int n;                    // transform length

@@ -217,6 +217,12 @@ __device__ __forceinline__ cplx ld_stream(const cplx* p)
     asm volatile("ld.global.cs.v2.f64 {%0, %1}, [%2];\n" : "=d"(v.x), "=d"(v.y) : "l"(p));
     return v;
 }
+__device__ __forceinline__ double ld_stream(const double* p)
+{
+    double v;
+    asm volatile("ld.global.cs.f64 %0, [%1];\n" : "=d"(v) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ void st_stream(cplx* p, cplx v)
 {
     asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};\n" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");

@@ -75,6 +75,12 @@ enum { PF_Z = 1, PF_SWEEP_Y = 2, PF_SWEEP_X = 4, PF_FFT_Y = 8, PF_FFT_X = 16 };
 
 struct dgpe_handle {
     int nx, ny, nz, nzh, mode;
+    // DGPE_IMAG_RPSI (SV section 8f NEXT-2): mode is DGPE_IMAG, psi is nx*ny*nz plain doubles.  The x and y
+    // sweeps act on the real and the imaginary part alike (real coefficients), so they run unchanged on psi
+    // viewed as complex [nx][ny][nz/2]; nzc is that column count (nz in the complex modes).
+    bool rpsi = false;
+    int nzc = 0;
+    cplx* psi_wide = nullptr;        // observables of a real-valued psi: its complex copy (lazy, 16 N bytes)
     double dx, dy, dz, dt, gamma, nu, lambda, g, gdd;
     long long N;
     cudaStream_t stream = nullptr;
@@ -331,6 +337,8 @@ static int init_handle(dgpe_handle* h)
         const char* e = getenv("DGPE_GENERIC");
         h->force_generic = e && e[0] == '1';
         h->zfast = !h->force_generic && z_specialised(nz);
+        if (h->rpsi && !h->zfast)
+            return fail(DGPE_ERR_UNSUPPORTED, "DGPE_IMAG_RPSI needs one of the specialised z lengths (nz = %d is not)", nz);
         const char* pf = getenv("DGPE_PREFETCH");
         if (pf && pf[0]) h->prefetch = atoi(pf);
         const char* tm = getenv("DGPE_TMA");
@@ -452,10 +460,16 @@ extern "C" dgpe_handle* dgpe_create(int nx, int ny, int nz, double dx, double dy
         fail(DGPE_ERR_ARG, "dx, dy, dz, dt must be positive and finite");
         return nullptr;
     }
-    if (mode != DGPE_IMAG && mode != DGPE_REAL) { fail(DGPE_ERR_ARG, "mode %d is neither DGPE_IMAG nor DGPE_REAL", mode); return nullptr; }
+    if (mode != DGPE_IMAG && mode != DGPE_REAL && mode != DGPE_IMAG_RPSI) {
+        fail(DGPE_ERR_ARG, "mode %d is none of DGPE_IMAG, DGPE_REAL, DGPE_IMAG_RPSI", mode);
+        return nullptr;
+    }
     dgpe_handle* h = new (std::nothrow) dgpe_handle();
     if (!h) { fail(DGPE_ERR_NOMEM, "host allocation failed"); return nullptr; }
-    h->nx = nx; h->ny = ny; h->nz = nz; h->nzh = nz / 2 + 1; h->mode = mode;
+    h->nx = nx; h->ny = ny; h->nz = nz; h->nzh = nz / 2 + 1;
+    h->rpsi = mode == DGPE_IMAG_RPSI;
+    h->mode = h->rpsi ? DGPE_IMAG : mode;
+    h->nzc = h->rpsi ? nz / 2 : nz;
     h->dx = dx; h->dy = dy; h->dz = dz; h->dt = dt;
     h->gamma = gamma; h->nu = nu; h->lambda = lambda; h->g = g; h->gdd = gdd;
     h->N = (long long)nx * ny * nz;
@@ -539,9 +553,9 @@ static void fill_chunk_tabs(const AxisSweep& S, bool use, ChunkTabs<CT, LC>* P)
 constexpr int Z_MAIN_WARPS = 1;      // warps per CTA of k_z_main: one, so that a finished line frees its slot at once
 
 template <int NZ>
-constexpr int z_main_minb(bool use_a, bool use_b)
+constexpr int z_main_minb(bool use_a, bool use_b, int a_size)
 {
-    const int per_cta = Z_MAIN_WARPS * ZGeom<NZ>::LPW * ((use_a ? ZGeom<NZ>::A_ELEMS : 0) + (use_b ? ZGeom<NZ>::B_ELEMS : 0)) * 16 + 1024;
+    const int per_cta = Z_MAIN_WARPS * ZGeom<NZ>::LPW * ((use_a ? ZGeom<NZ>::A_ELEMS * a_size : 0) + (use_b ? ZGeom<NZ>::B_ELEMS * 16 : 0)) + 1024;
     const int m = (227 * 1024) / per_cta, cap = 16 / Z_MAIN_WARPS;       // 16 warps per SM: 128 registers per thread
     return m < 1 ? 1 : (m > cap ? cap : m);
 }
@@ -552,22 +566,30 @@ static int launch_z_r2c_n(dgpe_handle* h, const cplx* psi)
     constexpr int WARPS = 1;                             // one warp per CTA: a finished line frees its slot at once
     constexpr int LINES = WARPS * ZGeom<NZ>::LPW;        // lines per CTA
     const size_t smem = (size_t)LINES * ZGeom<NZ>::B_ELEMS * sizeof(cplx);
-    auto kern = k_z_r2c<NZ, WARPS>;
+    const int nlines = h->nx * h->ny;
+    if (h->rpsi) {
+        auto kern = k_z_r2c<NZ, WARPS, double>;
+        int rc = kernel_setup((const void*)kern, 32 * WARPS, smem, nullptr);
+        if (rc) return rc;
+        kern<<<(nlines + LINES - 1) / LINES, 32 * WARPS, smem, h->stream>>>((const double*)psi, h->spec, nlines, h->tw_zh,
+                                                                            h->tw_split, h->scal);
+        return check_launch("k_z_r2c");
+    }
+    auto kern = k_z_r2c<NZ, WARPS, cplx>;
     int rc = kernel_setup((const void*)kern, 32 * WARPS, smem, nullptr);
     if (rc) return rc;
-    const int nlines = h->nx * h->ny;
     kern<<<(nlines + LINES - 1) / LINES, 32 * WARPS, smem, h->stream>>>(psi, h->spec, nlines, h->tw_zh, h->tw_split, h->scal);
     return check_launch("k_z_r2c");
 }
 
-template <int NZ, typename CT, int SPEC, bool SWEEP, bool CONSTTAB>
+template <int NZ, typename CT, typename DT, int SPEC, bool SWEEP, bool CONSTTAB>
 static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
 {
     constexpr int WARPS = Z_MAIN_WARPS, LC = ZGeom<NZ>::LC, LINES = WARPS * ZGeom<NZ>::LPW;
     constexpr bool USE_A = SPEC != ZS_PHI, USE_B = SPEC != ZS_NONE;
-    constexpr int MINB = z_main_minb<NZ>(USE_A, USE_B);
-    const size_t smem = (size_t)LINES * ((USE_A ? ZGeom<NZ>::A_ELEMS : 0) + (USE_B ? ZGeom<NZ>::B_ELEMS : 0)) * sizeof(cplx);
-    auto kern = k_z_main<NZ, CT, SPEC, SWEEP, CONSTTAB, WARPS, MINB>;
+    constexpr int MINB = z_main_minb<NZ>(USE_A, USE_B, (int)sizeof(DT));
+    const size_t smem = (size_t)LINES * ((USE_A ? ZGeom<NZ>::A_ELEMS * sizeof(DT) : 0) + (USE_B ? ZGeom<NZ>::B_ELEMS * sizeof(cplx) : 0));
+    auto kern = k_z_main<NZ, CT, DT, SPEC, SWEEP, CONSTTAB, WARPS, MINB>;
     int ctas_per_sm = 0;
     int rc = kernel_setup((const void*)kern, 32 * WARPS, smem, &ctas_per_sm);
     if (rc) return rc;
@@ -588,17 +610,17 @@ static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
     Z.dz = h->dz; Z.lam2 = h->lambda * h->lambda;
     Z.scal = h->scal; Z.tw = h->tw_zh; Z.tws = h->tw_split; Z.phi_out = phi_out;
     Z.pf_lines = (h->prefetch & PF_Z) ? h->pf_mult * ctas_per_sm * h->num_sms * LINES : 0;
-    kern<<<(Z.nlines + LINES - 1) / LINES, 32 * WARPS, smem, h->stream>>>(psi, h->spec, Z, T, P);
+    kern<<<(Z.nlines + LINES - 1) / LINES, 32 * WARPS, smem, h->stream>>>((DT*)psi, h->spec, Z, T, P);
     return check_launch("k_z_main");
 }
 
-template <int NZ, typename CT, int SPEC, bool SWEEP>
+template <int NZ, typename CT, typename DT, int SPEC, bool SWEEP>
 static int launch_z_main_n(dgpe_handle* h, cplx* psi, double* phi_out)
 {
     if constexpr (SWEEP) {
-        if (h->sw[2].consttab) return launch_z_main_c<NZ, CT, SPEC, true, true>(h, psi, phi_out);
+        if (h->sw[2].consttab) return launch_z_main_c<NZ, CT, DT, SPEC, true, true>(h, psi, phi_out);
     }
-    return launch_z_main_c<NZ, CT, SPEC, SWEEP, false>(h, psi, phi_out);
+    return launch_z_main_c<NZ, CT, DT, SPEC, SWEEP, false>(h, psi, phi_out);
 }
 
 // what: 0 = C2R + nonlinear, 1 = C2R + nonlinear + z sweep, 2 = z sweep only, 3 = C2R -> phi_out
@@ -606,14 +628,22 @@ template <int NZ>
 static int launch_z_main_nz(dgpe_handle* h, cplx* psi, int what, double* phi_out)
 {
     const bool imag = h->mode == DGPE_IMAG;
+    if (h->rpsi) {      // real-valued psi (psi points to doubles); ZS_PHI does not touch psi
+        switch (what) {
+            case 0: return launch_z_main_n<NZ, double, double, ZS_IMAG, false>(h, psi, nullptr);
+            case 1: return launch_z_main_n<NZ, double, double, ZS_IMAG, true>(h, psi, nullptr);
+            case 2: return launch_z_main_n<NZ, double, double, ZS_NONE, true>(h, psi, nullptr);
+            default: break;
+        }
+    }
     switch (what) {
-        case 0: return imag ? launch_z_main_n<NZ, double, ZS_IMAG, false>(h, psi, nullptr)
-                            : launch_z_main_n<NZ, cplx, ZS_REAL, false>(h, psi, nullptr);
-        case 1: return imag ? launch_z_main_n<NZ, double, ZS_IMAG, true>(h, psi, nullptr)
-                            : launch_z_main_n<NZ, cplx, ZS_REAL, true>(h, psi, nullptr);
-        case 2: return imag ? launch_z_main_n<NZ, double, ZS_NONE, true>(h, psi, nullptr)
-                            : launch_z_main_n<NZ, cplx, ZS_NONE, true>(h, psi, nullptr);
-        default: return launch_z_main_n<NZ, double, ZS_PHI, false>(h, psi, phi_out);
+        case 0: return imag ? launch_z_main_n<NZ, double, cplx, ZS_IMAG, false>(h, psi, nullptr)
+                            : launch_z_main_n<NZ, cplx, cplx, ZS_REAL, false>(h, psi, nullptr);
+        case 1: return imag ? launch_z_main_n<NZ, double, cplx, ZS_IMAG, true>(h, psi, nullptr)
+                            : launch_z_main_n<NZ, cplx, cplx, ZS_REAL, true>(h, psi, nullptr);
+        case 2: return imag ? launch_z_main_n<NZ, double, cplx, ZS_NONE, true>(h, psi, nullptr)
+                            : launch_z_main_n<NZ, cplx, cplx, ZS_NONE, true>(h, psi, nullptr);
+        default: return launch_z_main_n<NZ, double, cplx, ZS_PHI, false>(h, psi, phi_out);
     }
 }
 
@@ -870,7 +900,7 @@ static int launch_sweep_tma_s(dgpe_handle* h, cplx* psi, int axis, const LineMap
     int rc = kernel_setup((const void*)kern, thr, smem, &ctas_per_sm);
     if (rc) return rc;
     // psi viewed as doubles: x sweep {2 ny nz, nx, 1}, y sweep {2 nz, ny, nx}; box {16, box_rows, 1}
-    const cuuint64_t nx = h->nx, ny = h->ny, nz = h->nz;
+    const cuuint64_t nx = h->nx, ny = h->ny, nz = h->nzc;
     cuuint64_t dims[3], strides[2];
     if (axis == 0) { dims[0] = 2 * ny * nz; dims[1] = nx; dims[2] = 1; strides[0] = ny * nz * 16; strides[1] = nx * ny * nz * 16; }
     else { dims[0] = 2 * nz; dims[1] = ny; dims[2] = nx; strides[0] = nz * 16; strides[1] = ny * nz * 16; }
@@ -924,7 +954,7 @@ template <typename CT>
 static int launch_sweep_t(dgpe_handle* h, cplx* psi, int axis, bool fold)
 {
     const AxisSweep& S = h->sw[axis];
-    const int nx = h->nx, ny = h->ny, nz = h->nz;
+    const int nx = h->nx, ny = h->ny, nz = axis < 2 ? h->nzc : h->nz;      // x, y: complex columns along z
     SweepTables<CT> T;
     T.r = to_ct<CT>(S.r);
     T.omr2 = to_ct<CT>(1.0 - 2.0 * S.r);
@@ -1029,7 +1059,7 @@ static int one_step(dgpe_handle* h, cplx* psi, Mark mark)
 static int finish_steps(dgpe_handle* h, cplx* psi)
 {
     int rc;
-    k_scale<<<148 * 8, 256, 0, h->stream>>>(psi, h->N, h->scal);
+    k_scale<<<148 * 8, 256, 0, h->stream>>>(psi, h->rpsi ? h->N / 2 : h->N, h->scal);
     if ((rc = check_launch("k_scale"))) return rc;
     CU(cudaMemcpyAsync(h->h_out, h->scal, sizeof(double) * SC_COUNT, cudaMemcpyDeviceToHost, h->stream));
     return set_scal(h, 0);
@@ -1102,7 +1132,7 @@ extern "C" int dgpe_step_host(dgpe_handle* h, void* psi_host, int nsteps)
 {
     if (!h || !psi_host) return fail(DGPE_ERR_ARG, "NULL handle or psi");
     if (nsteps < 0) return fail(DGPE_ERR_ARG, "nsteps = %d < 0", nsteps);
-    const size_t bytes = sizeof(cplx) * (size_t)h->N;
+    const size_t bytes = (h->rpsi ? sizeof(double) : sizeof(cplx)) * (size_t)h->N;
     if (!h->psi_stage) {
         CU(cudaMalloc(&h->psi_stage, bytes));
         h->owned.push_back(h->psi_stage);
@@ -1167,7 +1197,8 @@ extern "C" const char* dgpe_kernel_name(const dgpe_handle* h, int k)
 extern "C" double dgpe_kernel_bytes(const dgpe_handle* h, int k)
 {
     if (!h) return 0.0;
-    const double N = (double)h->N, S = 16.0 * (double)h->nx * h->ny * h->nzh;
+    const double S = 16.0 * (double)h->nx * h->ny * h->nzh;
+    const double N = (h->rpsi ? 0.5 : 1.0) * (double)h->N;      // in units of 16 bytes of psi
     switch (k) {
         case 0: return 16.0 * N + S;       // read psi, write half-spectrum
         case 1: case 2: case 3: return 2.0 * S;
@@ -1223,8 +1254,42 @@ static int fetch(dgpe_handle* h, int count)
     return DGPE_OK;
 }
 
-static int moments(dgpe_handle* h, const void* psi)
+// Observables of a real-valued psi (DGPE_IMAG_RPSI; not on the timed path): psi is copied into a complex
+// array the handle owns and the handle behaves as a complex-psi one until the view is dropped.
+struct ComplexView {
+    dgpe_handle* h;
+    const void* psi;
+    bool widened = false;
+    int rc = DGPE_OK;
+    ComplexView(dgpe_handle* h_, const void* psi_) : h(h_), psi(psi_)
+    {
+        if (!h->rpsi) return;
+        if (!h->psi_wide) {
+            if (cudaMalloc(&h->psi_wide, sizeof(cplx) * (size_t)h->N) != cudaSuccess) {
+                cudaGetLastError();
+                rc = fail(DGPE_ERR_NOMEM, "no device memory for the complex copy of psi (%lld bytes)", 16LL * h->N);
+                return;
+            }
+            h->owned.push_back(h->psi_wide);
+        }
+        k_widen<<<148 * 8, 256, 0, h->stream>>>((const double*)psi_, h->psi_wide, h->N);
+        if ((rc = check_launch("k_widen"))) return;
+        psi = h->psi_wide;
+        h->rpsi = false;
+        h->nzc = h->nz;
+        widened = true;
+    }
+    ~ComplexView()
+    {
+        if (widened) { h->rpsi = true; h->nzc = h->nz / 2; }
+    }
+};
+
+static int moments(dgpe_handle* h, const void* psi_)
 {
+    ComplexView view(h, psi_);
+    if (view.rc) return view.rc;
+    const void* psi = view.psi;
     const int grid = std::min(h->nx * h->ny, 148 * 8);
     k_moments<<<grid, 256, 0, h->stream>>>((const cplx*)psi, obs_args(h, h->d_out));
     int rc = check_launch("k_moments");
@@ -1254,9 +1319,12 @@ extern "C" int dgpe_rms(dgpe_handle* h, const void* psi, double rms[4])
     return DGPE_OK;
 }
 
-extern "C" int dgpe_energy_terms(dgpe_handle* h, const void* psi, double out[4])
+extern "C" int dgpe_energy_terms(dgpe_handle* h, const void* psi_, double out[4])
 {
-    if (!h || !psi || !out) return fail(DGPE_ERR_ARG, "NULL argument");
+    if (!h || !psi_ || !out) return fail(DGPE_ERR_ARG, "NULL argument");
+    ComplexView view(h, psi_);
+    if (view.rc) return view.rc;
+    const void* psi = view.psi;
     int rc;
     if ((rc = launch_dipolar_spectrum(h, (const cplx*)psi))) return rc;
     if ((rc = launch_c2r(h, const_cast<cplx*>((const cplx*)psi), 2, h->d_out))) return rc;
@@ -1297,8 +1365,9 @@ extern "C" double dgpe_bytes_per_step(const dgpe_handle* h)
 {
     if (!h) return 0.0;
     const double N = (double)h->N, S = 16.0 * (double)h->nx * h->ny * h->nzh;
-    // K1 16N+S, K2 2S, K3 2S, K4 2S, K5 S+32N, three sweeps 32N each (model M1)
-    return 144.0 * N + 8.0 * S;
+    // K1 16N+S, K2 2S, K3 2S, K4 2S, K5 S+32N, three sweeps 32N each (model M1);
+    // real-valued psi: 8 bytes per point in every psi term, 72N + 8S (SV section 8f NEXT-2)
+    return (h->rpsi ? 72.0 : 144.0) * N + 8.0 * S;
 }
 
 extern "C" int dgpe_launches_per_step(const dgpe_handle* h)

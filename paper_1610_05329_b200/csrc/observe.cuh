@@ -13,6 +13,13 @@ struct ObsArgs {
     double* out;
 };
 
+// complex copy of a real-valued psi (DGPE_IMAG_RPSI observables)
+__global__ void k_widen(const double* __restrict__ src, cplx* __restrict__ dst, long long N)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < N; p += stride) dst[p] = mk(src[p], 0.0);
+}
+
 // out[0..3] = sum n, sum x^2 n, sum y^2 n, sum z^2 n      (n = |psi|^2)
 __global__ void k_moments(const cplx* __restrict__ psi, ObsArgs A)
 {

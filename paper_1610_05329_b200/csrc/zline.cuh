@@ -75,9 +75,11 @@ __device__ __forceinline__ cplx ct_zero(cplx) { return mk(0.0, 0.0); }
 // (Z_k - conj Z_{M-k}), k = 0..M, Z_M := Z_0.   tws[k] = exp(-2 pi i k/nz).
 // grid = ceil(nlines / (WARPS LPW)); block = 32*WARPS; dynamic shared memory = WARPS LPW B_ELEMS 16 bytes.
 // ------------------------------------------------------------------------------------------------
-template <int NZ, int WARPS>
+// DT = cplx: psi is complex (16 bytes per point); DT = double: real-valued psi of the imaginary-time
+// fast path (SV section 8f NEXT-2; 8 bytes per point, n = s2 psi^2).
+template <int NZ, int WARPS, typename DT>
 __global__ void __launch_bounds__(32 * WARPS)
-k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const cplx* __restrict__ tw,
+k_z_r2c(const DT* __restrict__ psi, cplx* __restrict__ spec, int nlines, const cplx* __restrict__ tw,
         const cplx* __restrict__ tws, const double* __restrict__ scal)
 {
     using G = ZGeom<NZ>;
@@ -92,7 +94,8 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
     double* Bd = reinterpret_cast<double*>(B);
     const double s2 = scal[SC_S2];
 
-    const cplx* p = psi + (long long)line * NZ;
+    constexpr bool RPSI = sizeof(DT) == sizeof(double);
+    const DT* p = psi + (long long)line * NZ;
     auto none = [](int) { return mk(0.0, 0.0); };
     auto keep = [&](int idx, cplx v) { B[PosPad::at(idx)] = v; };
     // z_m, m = lane + TL q, is exactly what butterfly `lane` of the first pass reads when that pass has
@@ -103,17 +106,26 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
         using P0 = CtPass<M, 0, false, false, TL>;
         static_assert(P0::NB == 1 && P0::R == M / TL && P0::Ns == 1, "first pass must be one butterfly per lane");
         P0 p0;
-        double4 w[P0::R];
+        if constexpr (RPSI) {
+            // the pair (psi_{2m}, psi_{2m+1}) is one 128-bit load: a warp reads 512 bytes contiguous
+            cplx w[P0::R];
 #pragma unroll
-        for (int q = 0; q < P0::R; ++q) {
-            const double* src = reinterpret_cast<const double*>(p + 2 * (lane + TL * q));
-            asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];\n"
-                         : "=d"(w[q].x), "=d"(w[q].y), "=d"(w[q].z), "=d"(w[q].w)
-                         : "l"(src));
+            for (int q = 0; q < P0::R; ++q) w[q] = ld_stream(reinterpret_cast<const cplx*>(p + 2 * (lane + TL * q)));
+#pragma unroll
+            for (int q = 0; q < P0::R; ++q) p0.v[0][q] = mk(s2 * (w[q].x * w[q].x), s2 * (w[q].y * w[q].y));
+        } else {
+            double4 w[P0::R];
+#pragma unroll
+            for (int q = 0; q < P0::R; ++q) {
+                const double* src = reinterpret_cast<const double*>(p + 2 * (lane + TL * q));
+                asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];\n"
+                             : "=d"(w[q].x), "=d"(w[q].y), "=d"(w[q].z), "=d"(w[q].w)
+                             : "l"(src));
+            }
+#pragma unroll
+            for (int q = 0; q < P0::R; ++q)
+                p0.v[0][q] = mk(s2 * (w[q].x * w[q].x + w[q].y * w[q].y), s2 * (w[q].z * w[q].z + w[q].w * w[q].w));
         }
-#pragma unroll
-        for (int q = 0; q < P0::R; ++q)
-            p0.v[0][q] = mk(s2 * (w[q].x * w[q].x + w[q].y * w[q].y), s2 * (w[q].z * w[q].z + w[q].w * w[q].w));
         p0.bfly(lane);
         if constexpr (P0::LAST) {
             p0.scatter(lane, keep);
@@ -123,11 +135,11 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
             ct_fft_range<M, false, false, TL, SyncWarp, PosPad, 1, L, false>(B, lane, true, tw, none, keep);
         }
     } else {
-        cplx a[G::NPER];
+        DT a[G::NPER];
 #pragma unroll
         for (int i = 0; i < G::NPER; ++i) {
             const int e = TL * i + lane;
-            a[i] = (NZ % TL == 0 || e < NZ) ? ld_stream(p + e) : mk(0.0, 0.0);
+            a[i] = (NZ % TL == 0 || e < NZ) ? ld_stream(p + e) : ct_zero(DT());
         }
 #pragma unroll
         for (int i = 0; i < G::NPER; ++i) {
@@ -170,7 +182,7 @@ k_z_r2c(const cplx* __restrict__ psi, cplx* __restrict__ spec, int nlines, const
 // Phi_{2m+1} = Im z_m.   H = V + g n + gdd Phi, n = s2 |psi|^2, V = (vx[i] + vy[j] + vz[k])/2.
 // Sweep: as sweep.cuh; lane l owns the unknowns 1 + l LC .. and keeps them in registers through the
 // forward elimination, the back substitution and the fix-up; the chunk outflows travel by shuffles.
-// grid = ceil(nlines / (WARPS LPW)); block = 32*WARPS; dynamic smem = WARPS LPW (A_ELEMS + B_ELEMS) 16 bytes.
+// grid = ceil(nlines / (WARPS LPW)); block = 32*WARPS; dynamic smem = WARPS LPW (A_ELEMS sizeof(DT) + B_ELEMS 16) bytes.
 // ------------------------------------------------------------------------------------------------
 enum { ZS_NONE = 0, ZS_IMAG = 1, ZS_REAL = 2, ZS_PHI = 3 };
 
@@ -202,9 +214,11 @@ __device__ __forceinline__ void bulk_store(void* gdst, const void* smem_src, uns
                  : "memory");
 }
 
-template <int NZ, typename CT, int SPEC, bool SWEEP, bool CONSTTAB, int WARPS, int MINB>
+// DT = cplx, or double for the real-valued psi of the imaginary-time fast path (CT = double, SPEC != ZS_REAL):
+// the line buffer A then holds nz doubles, and every quantity of the sweep is one double instead of two.
+template <int NZ, typename CT, typename DT, int SPEC, bool SWEEP, bool CONSTTAB, int WARPS, int MINB>
 __global__ void __launch_bounds__(32 * WARPS, MINB)
-k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, SweepTables<CT> T,
+k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, SweepTables<CT> T,
          const __grid_constant__ ChunkTabs<CT, ZGeom<NZ>::LC> P)
 {
     using G = ZGeom<NZ>;
@@ -218,25 +232,28 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
     const bool valid = line0 + team < Z.nlines;         // a team past the end works on the last line, stores nothing
     const int line = valid ? line0 + team : Z.nlines - 1;
     const int slot = warp * LPW + team;
-    constexpr int PER_LINE = (USE_A ? G::A_ELEMS : 0) + (SPEC != ZS_NONE ? G::B_ELEMS : 0);
-    cplx* A = reinterpret_cast<cplx*>(smem_raw) + (size_t)slot * PER_LINE;
-    cplx* B = A + (USE_A ? G::A_ELEMS : 0);
-    cplx* p = psi + (long long)line * NZ;
+    static_assert(sizeof(DT) == sizeof(cplx) || (sizeof(CT) == sizeof(double) && SPEC != ZS_REAL),
+                  "real-valued psi: imaginary time only");
+    constexpr unsigned A_BYTES = USE_A ? G::A_ELEMS * (unsigned)sizeof(DT) : 0u;      // a multiple of 16 (nz even)
+    constexpr unsigned PER_LINE = A_BYTES + (SPEC != ZS_NONE ? G::B_ELEMS * (unsigned)sizeof(cplx) : 0u);
+    DT* A = reinterpret_cast<DT*>(smem_raw + (size_t)slot * PER_LINE);
+    cplx* B = reinterpret_cast<cplx*>(smem_raw + (size_t)slot * PER_LINE + A_BYTES);
+    DT* p = psi + (long long)line * NZ;
 
     // ---- the psi line: one bulk copy, in flight while the spectrum is loaded, merged and transformed ----
     if constexpr (USE_A) {
         if (lane == 0) {
             mbar_init(&bars[slot], 1);
             mbar_fence_init();
-            mbar_expect_tx(&bars[slot], NZ * 16u);
-            bulk_load(A, p, NZ * 16u, &bars[slot]);
+            mbar_expect_tx(&bars[slot], A_BYTES);
+            bulk_load(A, p, A_BYTES, &bars[slot]);
         }
     }
     // ---- L2 prefetch for the warp that will run one residency later ----
     if (Z.pf_lines > 0 && line + Z.pf_lines < Z.nlines) {
         const char* pp = reinterpret_cast<const char*>(psi + (long long)(line + Z.pf_lines) * NZ);
         if constexpr (USE_A) {
-            for (int o = 128 * lane; o < NZ * 16; o += 128 * TL) prefetch_l2(pp + o);
+            for (int o = 128 * lane; o < (int)A_BYTES; o += 128 * TL) prefetch_l2(pp + o);
         }
         if constexpr (SPEC != ZS_NONE) {
             const char* ps = reinterpret_cast<const char*>(spec + (long long)(line + Z.pf_lines) * (M + 1));
@@ -307,8 +324,8 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         s2 = Z.scal[SC_S2];
         s1 = Z.scal[SC_S1];
     }
-    auto upd = [&](int e) -> cplx {
-        cplx a = A[e];
+    auto upd = [&](int e) -> DT {
+        DT a = A[e];
         if constexpr (SPEC == ZS_IMAG || SPEC == ZS_REAL) {
             const double z = (double)(e - NZ / 2) * Z.dz;          // R#6
             const double vz = Z.lam2 * z * z;
@@ -316,7 +333,7 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
             const double H = 0.5 * (vxy + vz) + Z.g * dens + Z.gdd * Bd[e];
             if constexpr (SPEC == ZS_IMAG) {
                 const double f = exp(-Z.dt * H) * s1;
-                a = mk(f * a.x, f * a.y);
+                a = coef_mul(f, a);
             } else {
                 double sn, cs;
                 sincos(Z.dt * H, &sn, &cs);
@@ -344,56 +361,55 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
         // (branch-free: every lane evaluates its LC updates on clamped indices and masks the ones past its
         // chunk or on an end node, so the exponentials of one lane interleave; the two halo values come
         // from the neighbouring lanes by shuffles -- every lane left of an active lane owns a full chunk)
-        cplx pv[LC + 2];
+        const DT zero = ct_zero(DT());
+        DT pv[LC + 2];
 #pragma unroll
         for (int i = 1; i <= LC; ++i) {
             const int j = s - 1 + i;
-            const cplx v = upd(min(j, NZ - 1));
-            const bool in = (j <= NZ - 2);
-            pv[i] = mk(in ? v.x : 0.0, in ? v.y : 0.0);
+            const DT v = upd(min(j, NZ - 1));
+            pv[i] = el_sel(j <= NZ - 2, v, zero);
         }
         {
-            const cplx up = shfl_c<TL>(pv[LC], (lane + TL - 1) & (TL - 1)), dn = shfl_c<TL>(pv[1], (lane + 1) & (TL - 1));
-            pv[0] = (lane == 0) ? mk(0.0, 0.0) : up;
-            pv[LC + 1] = (lane == TL - 1) ? mk(0.0, 0.0) : dn;
+            const DT up = shfl_ct<TL>(pv[LC], (lane + TL - 1) & (TL - 1)), dn = shfl_ct<TL>(pv[1], (lane + 1) & (TL - 1));
+            pv[0] = (lane == 0) ? zero : up;
+            pv[LC + 1] = (lane == TL - 1) ? zero : dn;
         }
-        cplx ev[LC];
-        cplx e = mk(0.0, 0.0);
+        DT ev[LC];
+        DT e = zero;
 #pragma unroll
         for (int i = 0; i < LC; ++i) {
             // inv_j (d_j + r e_{j-1}) = inv_j d_j + (-c_j) e_{j-1}: one dependent fma per unknown
-            cplx d = coef_mul(T.r, cadd(pv[i], pv[i + 2]));
+            DT d = coef_mul(T.r, cadd(pv[i], pv[i + 2]));
             d = coef_fma(T.omr2, pv[i + 1], d);
-            const cplx en = coef_fma(coef_neg(t_cc(i)), e, coef_mul(t_inv(i), d));
-            const bool on = i < cnt;
-            e = mk(on ? en.x : e.x, on ? en.y : e.y);
+            const DT en = coef_fma(coef_neg(t_cc(i)), e, coef_mul(t_inv(i), d));
+            e = el_sel(i < cnt, en, e);
             ev[i] = e;
         }
         // ---- B: forward inflow by a look-back over the lanes to the left ----
         const CT Ag = (lane < Gn) ? __ldg(&T.Ach[lane]) : ct_zero(CT());
         const CT Bg = (lane < Gn) ? __ldg(&T.Bch[lane]) : ct_zero(CT());
-        cplx ein = mk(0.0, 0.0);
+        DT ein = zero;
         for (int d = T.Kf; d >= 1; --d) {
             const int h = lane - d;
-            const cplx Eh = shfl_c<TL>(e, h & (TL - 1));
+            const DT Eh = shfl_ct<TL>(e, h & (TL - 1));
             const CT Ah = shfl_ct<TL>(Ag, h & (TL - 1));
             if (h >= 0) ein = coef_fma(Ah, ein, Eh);
         }
         // ---- C: local back substitution with zero inflow ----
-        cplx x = mk(0.0, 0.0);
+        DT x = zero;
 #pragma unroll
         for (int i = LC - 1; i >= 0; --i) {
             if (i < cnt) {
-                const cplx ee = coef_fma(t_F(i), ein, ev[i]);
+                const DT ee = coef_fma(t_F(i), ein, ev[i]);
                 x = coef_fma(coef_neg(t_cc(i)), x, ee);
                 ev[i] = x;
             }
         }
         // ---- D: backward inflow from the lanes to the right ----
-        cplx xin = mk(0.0, 0.0);
+        DT xin = zero;
         for (int d = T.Kb; d >= 1; --d) {
             const int h = lane + d;
-            const cplx Xh = shfl_c<TL>(x, h & (TL - 1));
+            const DT Xh = shfl_ct<TL>(x, h & (TL - 1));
             const CT Bh = shfl_ct<TL>(Bg, h & (TL - 1));
             if (h < Gn) xin = coef_fma(Bh, xin, Xh);
         }
@@ -402,8 +418,8 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
 #pragma unroll
         for (int i = 0; i < LC; ++i)
             if (i < cnt) A[s + i] = coef_fma(t_Gm(i), xin, ev[i]);
-        if (lane == 0) A[0] = mk(0.0, 0.0);
-        if (lane == TL - 1) A[NZ - 1] = mk(0.0, 0.0);
+        if (lane == 0) A[0] = zero;
+        if (lane == TL - 1) A[NZ - 1] = zero;
     } else {
         // nonlinear update only (dgpe_nonlinear): every point of the line, end nodes included
 #pragma unroll
@@ -417,7 +433,7 @@ k_z_main(cplx* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Swe
     fence_proxy_async();                                 // my writes -> visible to the async proxy
     __syncwarp();
     if (lane == 0 && valid) {
-        bulk_store(p, A, NZ * 16u);
+        bulk_store(p, A, A_BYTES);
         tma_store_commit();
         tma_store_wait_read<0>();                        // shared memory must outlive the copy
     }

@@ -36,7 +36,7 @@ def test_header_cites_the_paper_for_each_stage():
 
 @pytest.mark.parametrize("args,frag", [
     ((64, 64, 34, .1, .1, .1, .01, 1, 1, 1, 1, 1, 0), "2^a 3^b 5^c 7^d 11^e 13^f"),       # 34 = 2*17
-    ((64, 64, 54, .1, .1, .1, .01, 1, 1, 1, 1, 1, 2), "mode"),
+    ((64, 64, 54, .1, .1, .1, .01, 1, 1, 1, 1, 1, 3), "mode"),
     ((2, 64, 64, .1, .1, .1, .01, 1, 1, 1, 1, 1, 0), "< 4"),
     ((64, 64, 27, .1, .1, .1, .01, 1, 1, 1, 1, 1, 0), "even"),
     ((64, 76, 64, .1, .1, .1, .01, 1, 1, 1, 1, 1, 0), "2^a 3^b 5^c 7^d 11^e 13^f"),       # 76 = 4*19

@@ -318,6 +318,32 @@ def test_p8_real_time_norm_conservation(oracle):
 
 
 # ------------------------------------------------------------------------------------------
+# R#5: in imaginary time a real psi stays real, and the real and imaginary parts never mix
+# (every factor of the step is real).  This is what lets the library carry psi as plain doubles
+# (DGPE_IMAG_RPSI) and still be compared with this complex oracle.
+# ------------------------------------------------------------------------------------------
+
+def test_imaginary_time_keeps_a_real_psi_exactly_real(oracle):
+    cfg = inputs.scaled(inputs.CONFIGS["C1"], (16, 12, 20))
+    o = oracle.Oracle(*cfg.create_args())
+    psi = inputs.random_state(cfg.shape, 17)
+    re = np.ascontiguousarray(psi.real.astype(np.complex128))
+    for stage in (lambda a: o.nonlinear(a), lambda a: o.sweep(a, 0), lambda a: o.sweep(a, 1), lambda a: o.sweep(a, 2)):
+        a = re.copy()
+        stage(a)
+        assert np.all(a.imag == 0)
+    a = re.copy()
+    assert o.step(a, 5) == 0
+    assert np.all(a.imag == 0)
+    # the sweeps are real-linear: the sweep of the real part is the real part of the sweep
+    for axis in range(3):
+        full, part = psi.copy(), re.copy()
+        o.sweep(full, axis)
+        o.sweep(part, axis)
+        assert np.array_equal(full.real, part.real)
+
+
+# ------------------------------------------------------------------------------------------
 # P9: observables on a Gaussian (closed forms; spectrally accurate on these grids)
 # ------------------------------------------------------------------------------------------
 
