@@ -170,11 +170,12 @@ def run_reference(args, cfg):
 # ------------------------------------------------------------------------------------------------
 # the CUDA path
 # ------------------------------------------------------------------------------------------------
-def ncu_traffic(kernel_name):
+def ncu_traffic(kernel_name, rpsi=False):
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from
-    the committed `ncu --set full` capture, recorded in profiles/traffic.csv; else None."""
+    the committed `ncu --set full` capture, recorded in profiles/traffic.csv (traffic_rpsi.csv for the
+    real-valued path); else None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+        with open(os.path.join(ROOT, "profiles", "traffic_rpsi.csv" if rpsi else "traffic.csv")) as f:
             for line in f:
                 name, _, rest = line.rstrip("\n").partition(",")
                 if name == kernel_name:
@@ -239,7 +240,7 @@ def run_b200(args, cfg):
     top = max(kernels, key=lambda k: k["ms"])
     step_ms = sec_local / K * 1e3
     roofline = {"bound": "hbm", "kernel": top["name"], "achieved": top["GBps"], "peak": peak, "unit": "GB/s",
-                "frac": top["GBps"] / peak, "traffic": ncu_traffic(top["name"]), "peak_source": peak_src,
+                "frac": top["GBps"] / peak, "traffic": ncu_traffic(top["name"], rpsi) if cfg.name == "C4" else None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": top["bytes"], "kernel_ms": top["ms"],
                 "share_of_step": top["ms"] / sum(k["ms"] for k in kernels)}
     step_gbps = G.bytes_per_step / step_ms * 1e-6

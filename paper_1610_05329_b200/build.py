@@ -14,12 +14,13 @@ SOURCES = ["dgpe_api.cu"]
 DEPS = ["dgpe_api.cu", "common.cuh", "fft.cuh", "ctfft.cuh", "xyfft.cuh", "xysweep.cuh", "xysweep_tma.cuh", "xyfft_tma.cuh", "tma.cuh", "zline.cuh", "spectral.cuh", "sweep.cuh", "observe.cuh"]
 HEADER = os.path.join(os.path.dirname(HERE), "include", "dgpe.h")
 
+# (no -split-compile: measured on the B200, the kernels it produces are slower -- x sweep 0.83 -> 0.96 ms,
+# K3 0.67 -> 0.70 ms at 512^3 -- although it halves the build time)
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",
     "-shared", "-Xcompiler", "-fPIC",
     "-cudart", "static",
-    "-split-compile", "0",      # optimise the kernels of the one translation unit on all host cores
 ]
 
 

@@ -91,6 +91,9 @@ struct dgpe_handle {
     // it pays for the z-line kernels and the y axis; on the x axis (row stride ny*nz) it costs time
     int prefetch = PF_Z | PF_SWEEP_Y | PF_FFT_Y;
     bool use_tma_fft = true;         // DGPE_TMA_FFT=0: K2/K4 load and store through the threads (k_fft_xy)
+    // K3 on the TMA pipeline (k_fft_tma_xudd): measured 1.98 -> 1.45 ms at nx = 768 (one 768-thread CTA per SM
+    // otherwise), 0.67 -> 0.70 ms at nx = 512, so by default from nx = 640 up; DGPE_TMA_K3=0|1: never | every length
+    int use_tma_k3 = -1;
     bool use_tma_x = false;          // DGPE_TMA=2: TMA on the x axis at every length (A/B)
     bool use_tma = true;             // DGPE_TMA=0: the x/y sweeps load and store through the threads (k_sweep_xy)
     bool zfast = false;              // warp-per-line z kernels (zline.cuh) and the fused step order z, x, y
@@ -346,6 +349,8 @@ static int init_handle(dgpe_handle* h)
         h->use_tma_x = tm && tm[0] == '2';
         const char* tf = getenv("DGPE_TMA_FFT");
         h->use_tma_fft = h->use_tma && !(tf && tf[0] == '0');
+        const char* t3 = getenv("DGPE_TMA_K3");
+        h->use_tma_k3 = !h->use_tma ? 0 : (t3 && t3[0] == '1') ? 1 : (t3 && t3[0] == '0') ? 0 : -1;
         const char* gr = getenv("DGPE_GRAPH");
         h->use_graph = !(gr && gr[0] == '0');
         const char* pm = getenv("DGPE_PF_MULT");
@@ -550,13 +555,17 @@ static void fill_chunk_tabs(const AxisSweep& S, bool use, ChunkTabs<CT, LC>* P)
     }
 }
 
+#ifndef DGPE_ZCAP_RPSI
+#define DGPE_ZCAP_RPSI 20      // measured at 512^3: 16 -> 0.758 ms, 20 -> 0.733 ms, 24 -> 0.773 ms
+#endif
 constexpr int Z_MAIN_WARPS = 1;      // warps per CTA of k_z_main: one, so that a finished line frees its slot at once
 
 template <int NZ>
 constexpr int z_main_minb(bool use_a, bool use_b, int a_size)
 {
     const int per_cta = Z_MAIN_WARPS * ZGeom<NZ>::LPW * ((use_a ? ZGeom<NZ>::A_ELEMS * a_size : 0) + (use_b ? ZGeom<NZ>::B_ELEMS * 16 : 0)) + 1024;
-    const int m = (227 * 1024) / per_cta, cap = 16 / Z_MAIN_WARPS;       // 16 warps per SM: 128 registers per thread
+    // 16 warps per SM: 128 registers per thread; the real-valued sweep needs half the registers of the complex one
+    const int m = (227 * 1024) / per_cta, cap = (a_size == 8 ? DGPE_ZCAP_RPSI : 16) / Z_MAIN_WARPS;
     return m < 1 ? 1 : (m > cap ? cap : m);
 }
 
@@ -796,6 +805,48 @@ static int launch_fft_tma(dgpe_handle* h, bool inverse, bool* handled)
     }
 }
 
+// ---- K3 on the TMA pipeline (xyfft_tma.cuh k_fft_tma_xudd): the long x lines ----
+template <int N>
+static int launch_fft_tma_xudd_n(dgpe_handle* h)
+{
+    constexpr int NSTAGE = (3 * N * 128 <= 200 * 1024) ? 3 : 2;
+    auto kern = k_fft_tma_xudd<N, NSTAGE>;
+    const size_t smem = (size_t)NSTAGE * N * TILE_COLS * sizeof(cplx) + 128;
+    int rc = kernel_setup((const void*)kern, xy_threads<N>(), smem, nullptr);
+    if (rc) return rc;
+    const cuuint64_t nx = h->nx, ncols = (cuuint64_t)h->ny * h->nzh;
+    constexpr int nbox = tma_boxes(N);
+    static_assert(nbox > 0 && N % nbox == 0 && N / nbox <= 256, "line length must split into equal TMA boxes");
+    cuuint64_t dims[3] = {2 * ncols, nx, 1}, strides[2] = {ncols * 16, nx * ncols * 16};
+    cuuint32_t box[3] = {2 * TILE_COLS, (cuuint32_t)(N / nbox), 1}, estr[3] = {1, 1, 1};
+    CUtensorMap tmap;
+    CUresult cr = tensor_map_encoder()(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, h->spec, dims, strides, box, estr,
+                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                       CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (cr != CUDA_SUCCESS) return fail(DGPE_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)cr);
+    TmaWalk W;
+    W.n = N; W.box_rows = N / nbox;
+    W.tiles_per_batch = (int)((ncols + TILE_COLS - 1) / TILE_COLS);
+    W.ntiles = W.tiles_per_batch;
+    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 2.0 * 3.14159265358979323846264338327950288 / ((double)h->nx * h->dx), 1.0 / (double)h->N, 0};
+    kern<<<std::min(W.ntiles, h->num_sms), xy_threads<N>(), smem, h->stream>>>(tmap, W, h->tw_x, U, (int)ncols);
+    return check_launch("k_fft_tma_xudd");
+}
+
+static int launch_fft_tma_xudd(dgpe_handle* h, bool* handled)
+{
+    *handled = (h->use_tma_k3 == 1 || (h->use_tma_k3 < 0 && h->nx >= 640)) && tensor_map_encoder() != nullptr;
+    if (!*handled) return DGPE_OK;
+    switch (h->nx) {
+        case 384: return launch_fft_tma_xudd_n<384>(h);
+        case 480: return launch_fft_tma_xudd_n<480>(h);
+        case 512: return launch_fft_tma_xudd_n<512>(h);
+        case 640: return launch_fft_tma_xudd_n<640>(h);
+        case 768: return launch_fft_tma_xudd_n<768>(h);
+        default: *handled = false; return DGPE_OK;
+    }
+}
+
 static int launch_fft_y(dgpe_handle* h, bool inverse)
 {
     const int nx = h->nx, ny = h->ny, nzh = h->nzh;
@@ -827,7 +878,9 @@ static int launch_fft_x_udd(dgpe_handle* h)
     LineMap mx{nx, ny * nzh, 0, 1, (long long)ny * nzh};
     if (!h->force_generic) {
         bool handled = false;
-        int rc = launch_fft_xy<FFT_X_UDD>(h, nx, mx, 1, h->tw_x, &handled);
+        int rc = launch_fft_tma_xudd(h, &handled);
+        if (rc || handled) return rc;
+        rc = launch_fft_xy<FFT_X_UDD>(h, nx, mx, 1, h->tw_x, &handled);
         if (rc || handled) return rc;
     }
     const int tx = threads_for(h->plan_x.nbf);
@@ -973,7 +1026,9 @@ static int launch_sweep_t(dgpe_handle* h, cplx* psi, int axis, bool fold)
         // 0.75 vs 0.83 ms) and both axes for the long lines whose thread-loading CTAs are few and large
         // (768: 1.7 vs 2.3 ms).  On the x axis at n = 512 (rows ny*nz*16 bytes apart, one page each) it is
         // slower (0.94 vs 0.83 ms), and so it is for the short lines (256^3: 0.19 vs 0.11 ms).
-        const bool want_tma = (axis == 1 && m.n >= 384) || S.G > 64 || (h->use_tma_x);
+        // Real-valued psi: the complex rows of the x axis are ny*nz*8 bytes apart, and there the TMA walk wins
+        // on the x axis too (512^3: 0.39 vs 0.48 ms).
+        const bool want_tma = (axis == 1 && m.n >= 384) || S.G > 64 || (h->use_tma_x) || (h->rpsi && m.n >= 384);
         if (want_tma && tma_sweep_ok(h, m, S, &box_rows, &nstage))
             return S.consttab ? launch_sweep_tma<CT, true>(h, psi, axis, m, box_rows, nstage, thr, T, F, S)
                               : launch_sweep_tma<CT, false>(h, psi, axis, m, box_rows, nstage, thr, T, F, S);

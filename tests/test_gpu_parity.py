@@ -282,6 +282,28 @@ def test_kernel_variants_agree(gpu, monkeypatch, mode, env):
     assert float((alt - ref).abs().max()) <= 1e-13
 
 
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("nx", [384, 480, 512, 640])
+def test_k3_tma_pipeline_agrees(gpu, oracle, monkeypatch, nx, mode):
+    """K3 (FFT_x, Udd~, IFFT_x) has a thread-loading and a TMA-pipelined kernel (the default from nx = 640 up,
+    DESIGN.md section 6): each forced in turn gives the same Phi, and that Phi is the oracle's."""
+    shape = (nx, 12, 64)            # 12 * 33 = 396 flattened (ky, kz) columns: a ragged last tile (396 = 49 * 8 + 4)
+    args = (*shape, 0.3, 0.25, 0.2, 0.004, 1.0, 0.7, 1.3, 5.0, 3.0, mode)
+    psi = inputs.random_state(shape, 23) * 0.3
+    ref = oracle.Oracle(*args).dipolar(np.ascontiguousarray(psi.real ** 2 + psi.imag ** 2))
+    out = []
+    for val in ("0", "1"):
+        monkeypatch.setenv("DGPE_TMA_K3", val)
+        G = gpu.Dgpe(*args)
+        out.append(G.dipolar(dev(psi)).cpu().numpy())
+        assert np.max(np.abs(out[-1] - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref))), val
+        t = dev(psi)
+        G.step(t, 3)
+        out.append(t.cpu().numpy())
+    assert np.max(np.abs(out[0] - out[2])) <= 1e-13
+    assert np.max(np.abs(out[1] - out[3])) <= 1e-13
+
+
 def test_two_handles_on_two_streams(gpu):
     """Handles are independent: two of them stepping different states on two non-default streams at once
     give bit for bit what each gives alone on the default stream (CUDA graph replays included)."""
