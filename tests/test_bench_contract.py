@@ -29,6 +29,8 @@ def test_traffic_table_names_the_kernels_of_the_step():
     for name in ("K1 dens_r2c(z)", "K3 fft_x*Udd*ifft_x", "K5+K8 c2r(z)+nonlinear+sweep_z", "K7 sweep_y(+norm)"):
         t = bench.ncu_traffic(name)
         assert t is not None and 1e9 < t < 1e10, name
+        r = bench.ncu_traffic(name, rpsi=True)             # the real-valued path has its own capture
+        assert r is not None and 1e9 < r <= t, name
     assert bench.ncu_traffic("no such kernel") is None
     peak, src = bench.load_peaks()
     assert 3000 < peak < 9000 and ("measured" in src or "fallback" in src)
