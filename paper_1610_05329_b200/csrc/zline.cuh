@@ -101,26 +101,32 @@ k_z_r2c(const DT* __restrict__ psi, cplx* __restrict__ spec, int nlines, const c
     // z_m, m = lane + TL q, is exactly what butterfly `lane` of the first pass reads when that pass has
     // radix M/TL: then each lane loads its pairs (psi_{2m}, psi_{2m+1}) with one 256-bit load -- a warp
     // reads 1 KB contiguous -- and the densities go from registers straight into the pass
-    constexpr bool FIRST_IN_REGS = (M % TL == 0) && (ct::radix_at(M, 0, false) == M / TL);
+    // (also when the first pass has fewer butterflies than the team has lanes -- nz = 480: 30 radix-8
+    // butterflies -- the lanes past the last butterfly then sit the first pass out)
+    using P0 = CtPass<M, 0, false, false, TL>;
+    constexpr bool FIRST_IN_REGS = P0::NB == 1 && P0::Ns == 1;
     if constexpr (FIRST_IN_REGS) {
-        using P0 = CtPass<M, 0, false, false, TL>;
-        static_assert(P0::NB == 1 && P0::R == M / TL && P0::Ns == 1, "first pass must be one butterfly per lane");
+        constexpr int NB0 = P0::NBUT;                    // butterfly `lane` reads z_m, m = lane + NB0 q
+        const bool mine = P0::EXACT || lane < NB0;
         P0 p0;
         if constexpr (RPSI) {
             // the pair (psi_{2m}, psi_{2m+1}) is one 128-bit load: a warp reads 512 bytes contiguous
             cplx w[P0::R];
 #pragma unroll
-            for (int q = 0; q < P0::R; ++q) w[q] = ld_stream(reinterpret_cast<const cplx*>(p + 2 * (lane + TL * q)));
+            for (int q = 0; q < P0::R; ++q)
+                w[q] = mine ? ld_stream(reinterpret_cast<const cplx*>(p + 2 * (lane + NB0 * q))) : mk(0.0, 0.0);
 #pragma unroll
             for (int q = 0; q < P0::R; ++q) p0.v[0][q] = mk(s2 * (w[q].x * w[q].x), s2 * (w[q].y * w[q].y));
         } else {
             double4 w[P0::R];
 #pragma unroll
             for (int q = 0; q < P0::R; ++q) {
-                const double* src = reinterpret_cast<const double*>(p + 2 * (lane + TL * q));
-                asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];\n"
-                             : "=d"(w[q].x), "=d"(w[q].y), "=d"(w[q].z), "=d"(w[q].w)
-                             : "l"(src));
+                const double* src = reinterpret_cast<const double*>(p + 2 * (lane + NB0 * q));
+                w[q] = make_double4(0.0, 0.0, 0.0, 0.0);
+                if (mine)
+                    asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];\n"
+                                 : "=d"(w[q].x), "=d"(w[q].y), "=d"(w[q].z), "=d"(w[q].w)
+                                 : "l"(src));
             }
 #pragma unroll
             for (int q = 0; q < P0::R; ++q)
@@ -265,18 +271,22 @@ k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Sweep
         // ---- Hermitian merge straight from global memory ----
         // Z_k, k = lane + TL t, is exactly what butterfly `lane` of the first inverse pass reads when that
         // pass has radix M/TL: then the merged values go from registers straight into the pass
-        constexpr bool FIRST_IN_REGS = (M % TL == 0) && (ct::radix_at(M, 0, false) == M / TL);
+        // (or fewer butterflies than lanes: the bins are then dealt out with the butterfly count as the stride)
+        using P0 = CtPass<M, 0, true, false, TL>;
+        constexpr bool FIRST_IN_REGS = P0::NB == 1 && P0::Ns == 1;
+        constexpr int KSTR = FIRST_IN_REGS ? P0::NBUT : TL;       // lane's bins: k = lane + KSTR t
+        constexpr int KCNT = FIRST_IN_REGS ? P0::R : G::KPER;
         const cplx* in = spec + (long long)line * (M + 1);
-        cplx xa[G::KPER], xb[G::KPER];
+        cplx xa[KCNT], xb[KCNT];
 #pragma unroll
-        for (int t = 0; t < G::KPER; ++t) {
-            const int k = min(lane + TL * t, M - 1);              // (bins past M-1: loaded twice, never stored)
+        for (int t = 0; t < KCNT; ++t) {
+            const int k = min(lane + KSTR * t, M - 1);            // (bins past M-1: loaded twice, never stored)
             xa[t] = ld_stream(in + k);
             xb[t] = ld_stream(in + (M - k));
         }
 #pragma unroll
-        for (int t = 0; t < G::KPER; ++t) {
-            const int k = min(lane + TL * t, M - 1);
+        for (int t = 0; t < KCNT; ++t) {
+            const int k = min(lane + KSTR * t, M - 1);
             const cplx w = cconj(__ldg(&Z.tws[k]));               // e^{+2 pi i k/nz}
             const cplx cb = cconj(xb[t]);
             const cplx s = cadd(xa[t], cb), d = csub(xa[t], cb);
@@ -290,8 +300,6 @@ k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Sweep
         };
         auto none = [](int) { return mk(0.0, 0.0); };
         if constexpr (FIRST_IN_REGS) {
-            using P0 = CtPass<M, 0, true, false, TL>;
-            static_assert(P0::NB == 1 && P0::R == M / TL && P0::Ns == 1, "first pass must be one butterfly per lane");
             P0 p0;
 #pragma unroll
             for (int q = 0; q < P0::R; ++q) p0.v[0][q] = xa[q];
