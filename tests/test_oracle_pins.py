@@ -488,3 +488,20 @@ def test_create_rejects_bad_arguments(oracle):
         args[pos] = bad
         with pytest.raises(ValueError):
             oracle.Oracle(*args)
+
+
+# ------------------------------------------------------------------------------------------
+# input recipe: what `bench.py --rpsi` and tests/test_gpu_rpsi.py rely on
+# ------------------------------------------------------------------------------------------
+
+def test_imaginary_time_initial_states_are_real_normalised_and_zero_faced():
+    for name, shape in (("C1", (64, 64, 64)), ("C2", (32, 48, 64)), ("C4", (48, 32, 64))):
+        cfg = inputs.CONFIGS[name] if inputs.CONFIGS[name].shape == shape else inputs.scaled(inputs.CONFIGS[name], shape)
+        psi = inputs.initial_state(cfg)
+        assert psi.dtype == np.complex128 and psi.shape == shape
+        assert np.all(psi.imag == 0)                      # Gaussian x (1 + noise): real, so the real-valued path takes it as is
+        assert abs(np.sum(np.abs(psi) ** 2) * cfg.d[0] * cfg.d[1] * cfg.d[2] - 1) <= 1e-13
+        for face in (psi[0], psi[-1], psi[:, 0], psi[:, -1], psi[:, :, 0], psi[:, :, -1]):
+            assert np.all(face == 0)
+    c5 = inputs.initial_state(inputs.scaled(inputs.CONFIGS["C5"], (24, 24, 12)))
+    assert np.any(c5.imag != 0)                           # the seeded phase field makes C5 genuinely complex
