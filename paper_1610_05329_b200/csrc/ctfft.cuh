@@ -25,7 +25,8 @@ __host__ __device__ constexpr int pick(int m)
 // 320, 384 (M = 96, 160, 192), so that their first pass is one butterfly per lane, fed from registers
 // with every lane busy (zline.cuh).  Any radix order is a valid transform; the x/y kernels of the same
 // lengths simply use the same plan.
-__host__ __device__ constexpr int first_of(int n) { return n == 192 ? 6 : n == 160 ? 5 : n == 96 ? 3 : 0; }
+// (250 = nz/2 at nz = 500: radix 5 first gives 50 butterflies, two per lane, instead of 125 of radix 2)
+__host__ __device__ constexpr int first_of(int n) { return n == 192 ? 6 : n == 160 ? 5 : n == 96 ? 3 : n == 250 ? 5 : 0; }
 __host__ __device__ constexpr int npass(int n)
 {
     int c = 0;

@@ -102,35 +102,49 @@ k_z_r2c(const DT* __restrict__ psi, cplx* __restrict__ spec, int nlines, const c
     // radix M/TL: then each lane loads its pairs (psi_{2m}, psi_{2m+1}) with one 256-bit load -- a warp
     // reads 1 KB contiguous -- and the densities go from registers straight into the pass
     // (also when the first pass has fewer butterflies than the team has lanes -- nz = 480: 30 radix-8
-    // butterflies -- the lanes past the last butterfly then sit the first pass out)
+    // butterflies -- the lanes past the last butterfly then sit the first pass out; and with two butterflies
+    // per lane, j = lane and lane + TL, when it has more than the team has lanes -- nz = 500, 640, 768: measured
+    // at 256 x 256 x nz, complex psi 0.264 -> 0.221 ms (500), 0.234 -> 0.212 (640), but 0.236 -> 0.297 (768);
+    // real-valued psi 0.209 -> 0.183, 0.175 -> 0.155, 0.286 -> 0.199)
     using P0 = CtPass<M, 0, false, false, TL>;
-    constexpr bool FIRST_IN_REGS = P0::NB == 1 && P0::Ns == 1;
+    constexpr bool FIRST_IN_REGS = P0::Ns == 1 && (P0::NB == 1 || (P0::NB == 2 && (RPSI || NZ <= 640)));
     if constexpr (FIRST_IN_REGS) {
-        constexpr int NB0 = P0::NBUT;                    // butterfly `lane` reads z_m, m = lane + NB0 q
-        const bool mine = P0::EXACT || lane < NB0;
+        constexpr int NB0 = P0::NBUT, NBU = P0::NB;      // butterfly j reads z_m, m = j + NB0 q
         P0 p0;
         if constexpr (RPSI) {
             // the pair (psi_{2m}, psi_{2m+1}) is one 128-bit load: a warp reads 512 bytes contiguous
-            cplx w[P0::R];
+            cplx w[NBU][P0::R];
 #pragma unroll
-            for (int q = 0; q < P0::R; ++q)
-                w[q] = mine ? ld_stream(reinterpret_cast<const cplx*>(p + 2 * (lane + NB0 * q))) : mk(0.0, 0.0);
+            for (int u = 0; u < NBU; ++u)
 #pragma unroll
-            for (int q = 0; q < P0::R; ++q) p0.v[0][q] = mk(s2 * (w[q].x * w[q].x), s2 * (w[q].y * w[q].y));
+                for (int q = 0; q < P0::R; ++q) {
+                    const int j = lane + u * TL;
+                    w[u][q] = (P0::EXACT || j < NB0) ? ld_stream(reinterpret_cast<const cplx*>(p + 2 * (j + NB0 * q))) : mk(0.0, 0.0);
+                }
+#pragma unroll
+            for (int u = 0; u < NBU; ++u)
+#pragma unroll
+                for (int q = 0; q < P0::R; ++q) p0.v[u][q] = mk(s2 * (w[u][q].x * w[u][q].x), s2 * (w[u][q].y * w[u][q].y));
         } else {
-            double4 w[P0::R];
+            double4 w[NBU][P0::R];
 #pragma unroll
-            for (int q = 0; q < P0::R; ++q) {
-                const double* src = reinterpret_cast<const double*>(p + 2 * (lane + NB0 * q));
-                w[q] = make_double4(0.0, 0.0, 0.0, 0.0);
-                if (mine)
-                    asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];\n"
-                                 : "=d"(w[q].x), "=d"(w[q].y), "=d"(w[q].z), "=d"(w[q].w)
-                                 : "l"(src));
-            }
+            for (int u = 0; u < NBU; ++u)
 #pragma unroll
-            for (int q = 0; q < P0::R; ++q)
-                p0.v[0][q] = mk(s2 * (w[q].x * w[q].x + w[q].y * w[q].y), s2 * (w[q].z * w[q].z + w[q].w * w[q].w));
+                for (int q = 0; q < P0::R; ++q) {
+                    const int j = lane + u * TL;
+                    const double* src = reinterpret_cast<const double*>(p + 2 * (j + NB0 * q));
+                    w[u][q] = make_double4(0.0, 0.0, 0.0, 0.0);
+                    if (P0::EXACT || j < NB0)
+                        asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];\n"
+                                     : "=d"(w[u][q].x), "=d"(w[u][q].y), "=d"(w[u][q].z), "=d"(w[u][q].w)
+                                     : "l"(src));
+                }
+#pragma unroll
+            for (int u = 0; u < NBU; ++u)
+#pragma unroll
+                for (int q = 0; q < P0::R; ++q)
+                    p0.v[u][q] = mk(s2 * (w[u][q].x * w[u][q].x + w[u][q].y * w[u][q].y),
+                                    s2 * (w[u][q].z * w[u][q].z + w[u][q].w * w[u][q].w));
         }
         p0.bfly(lane);
         if constexpr (P0::LAST) {
@@ -273,20 +287,26 @@ k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Sweep
         // pass has radix M/TL: then the merged values go from registers straight into the pass
         // (or fewer butterflies than lanes: the bins are then dealt out with the butterfly count as the stride)
         using P0 = CtPass<M, 0, true, false, TL>;
+        // (one butterfly per lane only: with two, the 2 x 2 R merged bins in registers slow this kernel down --
+        // measured at nz = 500, 640, 768)
         constexpr bool FIRST_IN_REGS = P0::NB == 1 && P0::Ns == 1;
-        constexpr int KSTR = FIRST_IN_REGS ? P0::NBUT : TL;       // lane's bins: k = lane + KSTR t
-        constexpr int KCNT = FIRST_IN_REGS ? P0::R : G::KPER;
+        // lane's bins: t = u R + q -> k = (lane + u TL) + NBUT q (butterfly j = lane + u TL of the first pass), else k = lane + TL t
+        constexpr int KCNT = FIRST_IN_REGS ? P0::NB * P0::R : G::KPER;
+        auto bin = [&](int t) {
+            if constexpr (FIRST_IN_REGS) return min(lane + (t / P0::R) * TL + P0::NBUT * (t % P0::R), M - 1);
+            else return min(lane + TL * t, M - 1);                // (bins past M-1: loaded twice, never stored)
+        };
         const cplx* in = spec + (long long)line * (M + 1);
         cplx xa[KCNT], xb[KCNT];
 #pragma unroll
         for (int t = 0; t < KCNT; ++t) {
-            const int k = min(lane + KSTR * t, M - 1);            // (bins past M-1: loaded twice, never stored)
+            const int k = bin(t);
             xa[t] = ld_stream(in + k);
             xb[t] = ld_stream(in + (M - k));
         }
 #pragma unroll
         for (int t = 0; t < KCNT; ++t) {
-            const int k = min(lane + KSTR * t, M - 1);
+            const int k = bin(t);
             const cplx w = cconj(__ldg(&Z.tws[k]));               // e^{+2 pi i k/nz}
             const cplx cb = cconj(xb[t]);
             const cplx s = cadd(xa[t], cb), d = csub(xa[t], cb);
@@ -302,7 +322,9 @@ k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Sweep
         if constexpr (FIRST_IN_REGS) {
             P0 p0;
 #pragma unroll
-            for (int q = 0; q < P0::R; ++q) p0.v[0][q] = xa[q];
+            for (int u = 0; u < P0::NB; ++u)
+#pragma unroll
+                for (int q = 0; q < P0::R; ++q) p0.v[u][q] = xa[u * P0::R + q];
             p0.bfly(lane);
             if constexpr (P0::LAST) {
                 p0.scatter(lane, keep_phi);
