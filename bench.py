@@ -41,6 +41,7 @@ def parse():
     ap.add_argument("--rpsi", action="store_true",
                     help="imaginary-time configs: time the real-valued-psi path DGPE_IMAG_RPSI (SURVEY 8f NEXT-2); "
                          "not the headline, which stays complex psi as BASELINE.json states")
+    ap.add_argument("--opt", default="", help="dgpe_create_ex options for A/B runs, e.g. 'fused_fft=0,tma=0' (include/dgpe.h)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -209,7 +210,8 @@ def run_b200(args, cfg):
     rpsi = bool(args.rpsi)
     if rpsi and cfg.mode != 0:
         raise SystemExit("--rpsi needs an imaginary-time config")
-    G = binding.Dgpe(*mycfg.create_args()[:-1], binding.IMAG_RPSI if rpsi else mycfg.mode)
+    G = binding.Dgpe(*mycfg.create_args()[:-1], binding.IMAG_RPSI if rpsi else mycfg.mode,
+                     options=binding.parse_options(args.opt))
     state = inputs.initial_state(mycfg)
     if rpsi:
         import numpy as np

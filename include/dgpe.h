@@ -74,11 +74,40 @@ enum {
  *   g, gdd       contact and dipolar interaction strengths; dipoles polarised along z (R#2).
  *   mode         DGPE_IMAG, DGPE_REAL or DGPE_IMAG_RPSI.
  * Returns NULL on error (DGPE_ERR_ARG / UNSUPPORTED / NOMEM / CUDA in dgpe_last_error()).
- * Uses the current CUDA device; allocates 16*nx*ny*(nz/2+1) bytes plus O(nx+ny+nz) tables.
+ * Uses the current CUDA device, which the handle remembers: every later call with this handle returns DGPE_ERR_ARG
+ * if another device is current.  Allocates 16*nx*ny*(nz/2+1) bytes plus O(nx+ny+nz) tables.
  */
 #define DGPE_MAX_N 1024
 dgpe_handle* dgpe_create(int nx, int ny, int nz, double dx, double dy, double dz, double dt,
                          double gamma, double nu, double lambda, double g, double gdd, int mode);
+
+/*
+ * dgpe_create_ex -- dgpe_create with kernel-selection options, for A/B measurements and for the in-repo
+ * cross-checks of one kernel family against another (tests/test_gpu_parity.py test_kernel_variants_agree).
+ * Every field: -1 = the library's default (what dgpe_create uses; opt = NULL means all defaults).  The results
+ * are the same within rounding whatever the options; the library itself never reads the environment.
+ */
+typedef struct dgpe_options {
+    int generic;      /* 1: the runtime-plan (generic) kernels everywhere                                   */
+    int tma;          /* 0: x/y sweeps load and store through the threads; 2: TMA on the x axis as well     */
+    int tma_fft;      /* 0: K2/K4 through the threads (k_fft_xy) instead of the TMA pipeline                 */
+    int tma_k3;       /* 0 | 1: K3 never | always on the TMA pipeline (default: from nx = 640 up)           */
+    int graph;        /* 0: plain launches instead of replaying the captured one-step CUDA graph            */
+    int prefetch;     /* mask of kernel families with the L2 prefetch of the next residency:
+                         1 z lines, 2 y sweep, 4 x sweep, 8 y FFT, 16 x FFT                                 */
+    int pf_mult;      /* prefetch distance in units of one residency (default 1)                            */
+    int fused_fft;    /* 0: K2, K3, K4 as three launches; 1: as one persistent kernel over L2-resident kz
+                         slabs whenever the shape allows (default: when two slab groups fit L2)             */
+    int fused_group;  /* kz slabs per group of the fused kernel's queue (default: from the slab size)       */
+    int fused_sweep;  /* 0: x and y sweeps as two launches; 1: one persistent kernel over L2-resident z slabs */
+    int reserved[6];  /* set to -1 */
+} dgpe_options;
+dgpe_handle* dgpe_create_ex(int nx, int ny, int nz, double dx, double dy, double dz, double dt,
+                            double gamma, double nu, double lambda, double g, double gdd, int mode,
+                            const dgpe_options* opt);
+
+/* The DGPE_ERR_* code of this thread's last failed dgpe_create / dgpe_create_ex (DGPE_OK if it succeeded). */
+int dgpe_last_error_code(void);
 
 /* Frees the handle's device and host memory.  NULL is allowed. */
 void dgpe_destroy(dgpe_handle* h);

@@ -13,12 +13,41 @@ from . import build as _build
 IMAG, REAL, IMAG_RPSI = 0, 1, 2
 OK, ERR_ARG, ERR_CUDA, ERR_NOMEM, ERR_UNSUPPORTED, ERR_NONFINITE = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ("dgpe_create", "dgpe_destroy", "dgpe_set_stream", "dgpe_step", "dgpe_norm", "dgpe_chempot",
+EXPORTS = ("dgpe_create", "dgpe_create_ex", "dgpe_last_error_code", "dgpe_destroy", "dgpe_set_stream", "dgpe_step", "dgpe_norm", "dgpe_chempot",
            "dgpe_energy", "dgpe_rms", "dgpe_energy_terms", "dgpe_dipolar", "dgpe_nonlinear", "dgpe_sweep",
            "dgpe_step_host", "dgpe_step_profile", "dgpe_kernel_name", "dgpe_kernel_bytes",
            "dgpe_synchronize", "dgpe_bytes_per_step", "dgpe_launches_per_step", "dgpe_last_error")
 
 _lib = None
+
+# fields of dgpe_options (include/dgpe.h), in order; -1 = the library's default
+OPTION_FIELDS = ("generic", "tma", "tma_fft", "tma_k3", "graph", "prefetch", "pf_mult", "fused_fft", "fused_group",
+                 "fused_sweep")
+
+
+class DgpeOptions(C.Structure):
+    _fields_ = [(name, C.c_int) for name in OPTION_FIELDS] + [("reserved", C.c_int * 6)]
+
+    def __init__(self, **kw):
+        super().__init__()
+        for name in OPTION_FIELDS:
+            setattr(self, name, -1)
+        for i in range(6):
+            self.reserved[i] = -1
+        for name, val in kw.items():
+            if name not in OPTION_FIELDS:
+                raise KeyError(f"unknown dgpe option {name!r} (known: {OPTION_FIELDS})")
+            setattr(self, name, int(val))
+
+
+def parse_options(text):
+    """'generic=1,tma=0' -> dict, for command lines (bench.py --opt); the library reads no environment."""
+    out = {}
+    for item in (text or "").split(","):
+        if item.strip():
+            k, _, v = item.partition("=")
+            out[k.strip()] = int(v)
+    return out
 
 
 class DgpeError(RuntimeError):
@@ -36,6 +65,10 @@ def lib():
         vp, dp, ci, cd = C.c_void_p, C.POINTER(C.c_double), C.c_int, C.c_double
         L.dgpe_create.restype = vp
         L.dgpe_create.argtypes = [ci, ci, ci, cd, cd, cd, cd, cd, cd, cd, cd, cd, ci]
+        L.dgpe_create_ex.restype = vp
+        L.dgpe_create_ex.argtypes = [ci, ci, ci, cd, cd, cd, cd, cd, cd, cd, cd, cd, ci, C.POINTER(DgpeOptions)]
+        L.dgpe_last_error_code.restype = ci
+        L.dgpe_last_error_code.argtypes = []
         L.dgpe_destroy.restype = None
         L.dgpe_destroy.argtypes = [vp]
         L.dgpe_set_stream.argtypes = [vp, vp]
@@ -74,15 +107,21 @@ class Dgpe:
     """One dgpe_handle.  psi arguments are contiguous torch.complex128 CUDA tensors of shape (nx, ny, nz)
     (torch.float64 for mode IMAG_RPSI, the real-valued imaginary-time path)."""
 
-    def __init__(self, nx, ny, nz, dx, dy, dz, dt, gamma, nu, lam, g, gdd, mode, stream=None):
+    def __init__(self, nx, ny, nz, dx, dy, dz, dt, gamma, nu, lam, g, gdd, mode, stream=None, options=None):
+        """options: dict of dgpe_options fields (kernel selection for A/B runs and cross-checks) -> dgpe_create_ex."""
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1610_05329_b200 needs a CUDA device (no CPU fallback)")
         self.shape = (nx, ny, nz)
         self.mode = mode
         self.dtype = torch.float64 if mode == IMAG_RPSI else torch.complex128
-        self.h = lib().dgpe_create(nx, ny, nz, dx, dy, dz, dt, gamma, nu, lam, g, gdd, mode)
+        self.device = torch.device("cuda", torch.cuda.current_device())
+        if options:
+            opt = DgpeOptions(**options)
+            self.h = lib().dgpe_create_ex(nx, ny, nz, dx, dy, dz, dt, gamma, nu, lam, g, gdd, mode, C.byref(opt))
+        else:
+            self.h = lib().dgpe_create(nx, ny, nz, dx, dy, dz, dt, gamma, nu, lam, g, gdd, mode)
         if not self.h:
-            raise DgpeError(ERR_ARG, last_error())
+            raise DgpeError(lib().dgpe_last_error_code() or ERR_ARG, last_error())
         self.set_stream(stream if stream is not None else torch.cuda.current_stream())
 
     def close(self):
@@ -104,6 +143,8 @@ class Dgpe:
         if not (isinstance(psi, torch.Tensor) and psi.is_cuda and psi.dtype == self.dtype
                 and psi.is_contiguous() and tuple(psi.shape) == self.shape):
             raise TypeError(f"psi must be a contiguous CUDA {self.dtype} tensor of shape {self.shape}")
+        if psi.device != self.device:
+            raise TypeError(f"psi lives on {psi.device} but the handle was created on {self.device}")
         return C.c_void_p(psi.data_ptr())
 
     def step(self, psi, nsteps=1):

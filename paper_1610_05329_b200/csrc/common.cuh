@@ -36,6 +36,7 @@ __device__ __forceinline__ cplx coef_fma(cplx c, cplx b, cplx a)
 
 // Real-valued psi (imaginary time, SV section 8f NEXT-2): the same sweep arithmetic on plain doubles.
 __device__ __forceinline__ double cadd(double a, double b) { return a + b; }
+__device__ __forceinline__ double csub(double a, double b) { return a - b; }
 __device__ __forceinline__ double cabs2(double a) { return a * a; }
 __device__ __forceinline__ double coef_mul(double c, double v) { return c * v; }
 __device__ __forceinline__ double coef_fma(double c, double b, double a) { return fma(c, b, a); }

@@ -27,6 +27,7 @@
 #include "xysweep.cuh"
 #include "xysweep_tma.cuh"
 #include "xyfft_tma.cuh"
+#include "xyfft_fused.cuh"
 #include "zline.cuh"
 
 using namespace dgpe;
@@ -80,7 +81,6 @@ struct dgpe_handle {
     // viewed as complex [nx][ny][nz/2]; nzc is that column count (nz in the complex modes).
     bool rpsi = false;
     int nzc = 0;
-    cplx* psi_wide = nullptr;        // observables of a real-valued psi: its complex copy (lazy, 16 N bytes)
     double dx, dy, dz, dt, gamma, nu, lambda, g, gdd;
     long long N;
     cudaStream_t stream = nullptr;
@@ -97,6 +97,14 @@ struct dgpe_handle {
     bool use_tma_x = false;          // DGPE_TMA=2: TMA on the x axis at every length (A/B)
     bool use_tma = true;             // DGPE_TMA=0: the x/y sweeps load and store through the threads (k_sweep_xy)
     bool zfast = false;              // warp-per-line z kernels (zline.cuh) and the fused step order z, x, y
+    // K2 + K3 + K4 as one persistent kernel over L2-resident kz slabs (xyfft_fused.cuh): nx == ny, one of the
+    // specialised lengths, two slab groups fit L2.  DGPE_FUSED_FFT=0 keeps the three launches (A/B runs).
+    dgpe_options opt;                // as given to dgpe_create_ex (all -1 from dgpe_create)
+    int device = 0;                  // the CUDA device the handle lives on (current at creation)
+    bool fused_fft = false;
+    int fused_nslab = 0, fused_nunits = 0, fused_gs = 0;
+    int* fused_units = nullptr;          // device: queue order of the (phase, slab) units
+    unsigned int* fused_ctr = nullptr;   // device: queue head + 2 nslab tile counters
 
     cplx* spec = nullptr;                       // [nx][ny][nzh]
     FftPlan plan_x{}, plan_y{}, plan_zh{};      // transform lengths nx, ny, nz/2
@@ -116,13 +124,15 @@ struct dgpe_handle {
     bool use_graph = true;           // DGPE_GRAPH=0: plain launches
     bool warmed = false;             // one eager step has run (lazy per-kernel attribute setup done)
     cudaStream_t cap_stream = nullptr;
-    cudaGraphExec_t step_exec = nullptr;
-    cplx* step_exec_psi = nullptr;
+    // one instantiated graph per psi pointer, most recently used first (ping-pong buffers, dgpe_step after
+    // dgpe_step_host, ... keep their graphs)
+    std::vector<std::pair<cplx*, cudaGraphExec_t>> step_execs;
     std::vector<cudaEvent_t> prof_ev; // dgpe_step_profile
     std::vector<void*> owned;        // everything to cudaFree
 };
 
 static bool z_specialised(int nz);
+static bool fused_fft_supported(int nx, int ny);
 
 static int threads_for(int nbf)
 {
@@ -293,14 +303,6 @@ static size_t sweep_smem(int n, int G, bool zaxis)
     return sizeof(cplx) * ((size_t)n * (zaxis ? 9 : 8) + 2 * (size_t)G * TILE_COLS);
 }
 
-template <typename K>
-static int allow_smem(K kernel, size_t bytes)
-{
-    if (bytes > 227 * 1024) return fail(DGPE_ERR_UNSUPPORTED, "tile needs %zu bytes of shared memory", bytes);
-    CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-    return DGPE_OK;
-}
-
 // Per (kernel, device) setup that must precede a launch with more than 48 KB of dynamic shared memory,
 // and the resident CTAs per SM of that launch shape.  Cached: the kernels are launched thousands of
 // times; keyed by device so that one process may hold handles on several GPUs; guarded for threads.
@@ -309,6 +311,7 @@ static int kernel_setup(const void* func, int threads, size_t smem, int* ctas_pe
     static std::mutex mu;
     static std::map<std::pair<const void*, int>, size_t> allowed;                              // (kernel, device) -> opt-in bytes
     static std::map<std::tuple<const void*, int, int, size_t>, int> resident;                  // + (threads, bytes) -> CTAs per SM
+    if (smem > 227 * 1024) return fail(DGPE_ERR_UNSUPPORTED, "a kernel needs %zu bytes of shared memory", smem);
     int dev = 0;
     CU(cudaGetDevice(&dev));
     std::lock_guard<std::mutex> lock(mu);
@@ -336,25 +339,21 @@ static int init_handle(dgpe_handle* h)
     {
         int dev = 0;
         CU(cudaGetDevice(&dev));
+        h->device = dev;
         CU(cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev));
-        const char* e = getenv("DGPE_GENERIC");
-        h->force_generic = e && e[0] == '1';
+        // options (dgpe_create_ex; -1 = default): A/B switches and in-repo cross-checks, never read from the environment
+        const dgpe_options& o = h->opt;
+        h->force_generic = o.generic == 1;
         h->zfast = !h->force_generic && z_specialised(nz);
         if (h->rpsi && !h->zfast)
             return fail(DGPE_ERR_UNSUPPORTED, "DGPE_IMAG_RPSI needs one of the specialised z lengths (nz = %d is not)", nz);
-        const char* pf = getenv("DGPE_PREFETCH");
-        if (pf && pf[0]) h->prefetch = atoi(pf);
-        const char* tm = getenv("DGPE_TMA");
-        h->use_tma = !(tm && tm[0] == '0');
-        h->use_tma_x = tm && tm[0] == '2';
-        const char* tf = getenv("DGPE_TMA_FFT");
-        h->use_tma_fft = h->use_tma && !(tf && tf[0] == '0');
-        const char* t3 = getenv("DGPE_TMA_K3");
-        h->use_tma_k3 = !h->use_tma ? 0 : (t3 && t3[0] == '1') ? 1 : (t3 && t3[0] == '0') ? 0 : -1;
-        const char* gr = getenv("DGPE_GRAPH");
-        h->use_graph = !(gr && gr[0] == '0');
-        const char* pm = getenv("DGPE_PF_MULT");
-        if (pm && atoi(pm) > 0) h->pf_mult = atoi(pm);
+        if (o.prefetch >= 0) h->prefetch = o.prefetch;
+        h->use_tma = o.tma != 0;
+        h->use_tma_x = o.tma == 2;
+        h->use_tma_fft = h->use_tma && o.tma_fft != 0;
+        h->use_tma_k3 = !h->use_tma ? 0 : (o.tma_k3 == 1) ? 1 : (o.tma_k3 == 0) ? 0 : -1;
+        h->use_graph = o.graph != 0;
+        if (o.pf_mult > 0) h->pf_mult = o.pf_mult;
     }
 
     if ((rc = make_plan(h, nx, &h->plan_x, &h->tw_x, 128))) return rc;
@@ -423,54 +422,64 @@ static int init_handle(dgpe_handle* h)
     h->owned.push_back(h->d_out);
     CU(cudaMallocHost(&h->h_out, sizeof(double) * 16));
 
-    // shared-memory opt-in for every kernel that may exceed 48 KB
-    const size_t fft_xy = sizeof(cplx) * TILE_COLS * (size_t)std::max(nx, ny);
-    const size_t fft_z = sizeof(cplx) * TILE_COLS * (size_t)(M + 1);
-    if ((rc = allow_smem(k_fft_lines<false, 512>, fft_xy))) return rc;
-    if ((rc = allow_smem(k_fft_lines<true, 512>, fft_xy))) return rc;
-    if ((rc = allow_smem(k_fft_lines<false, 1024>, fft_xy))) return rc;
-    if ((rc = allow_smem(k_fft_lines<true, 1024>, fft_xy))) return rc;
-    if ((rc = allow_smem(k_fft_x_udd<512>, fft_xy))) return rc;
-    if ((rc = allow_smem(k_fft_x_udd<1024>, fft_xy))) return rc;
-    if ((rc = allow_smem(k_dens_r2c, fft_z))) return rc;
-    if ((rc = allow_smem(k_c2r_nonlin<0>, fft_z))) return rc;
-    if ((rc = allow_smem(k_c2r_nonlin<1>, fft_z))) return rc;
-    if ((rc = allow_smem(k_c2r_nonlin<2>, fft_z))) return rc;
-    if ((rc = allow_smem(k_c2r_nonlin<3>, fft_z))) return rc;
-    size_t sxy = std::max(sweep_smem(nx, h->sw[0].G, false), sweep_smem(ny, h->sw[1].G, false));
-    size_t sz = sweep_smem(nz, h->sw[2].G, true);
-    if (h->mode == DGPE_IMAG) {
-        if ((rc = allow_smem(k_sweep<double, false>, sxy))) return rc;
-        if ((rc = allow_smem(k_sweep<double, true>, sz))) return rc;
-    } else {
-        if ((rc = allow_smem(k_sweep<cplx, false>, sxy))) return rc;
-        if ((rc = allow_smem(k_sweep<cplx, true>, sz))) return rc;
+    // K2 + K3 + K4 through L2 (xyfft_fused.cuh): queue order of the (phase, slab) units,
+    //   A(g), C(g-1), B(g), A(g+1), C(g), B(g+1), ...   over groups g of `gs` neighbouring kz slabs,
+    // so that two groups are alive in L2 at a time and a phase's producer was handed out a whole phase earlier.
+    if (fused_fft_supported(nx, ny) && !h->force_generic && h->opt.fused_fft != 0) {
+        const int nslab = (nzh + TILE_COLS - 1) / TILE_COLS;
+        const double slab_bytes = (double)nx * ny * TILE_COLS * sizeof(cplx);
+        // group size: two groups within ~70 MB of the 126 MB L2 (one 33.5 MB slab per group at 512^2), and
+        // enough tiles per phase to fill the machine on the small grids
+        int gs = (int)(35.0e6 / slab_bytes);
+        gs = std::max(1, std::min(gs, nslab));
+        if (h->opt.fused_group > 0) gs = std::min(h->opt.fused_group, nslab);
+        if (2.0 * gs * slab_bytes <= 100.0e6 || h->opt.fused_fft == 1) {
+            std::vector<int> units;
+            const int G = (nslab + gs - 1) / gs;
+            auto emit = [&](int phase, int g) {
+                if (g < 0 || g >= G) return;
+                for (int sl = g * gs; sl < std::min(nslab, (g + 1) * gs); ++sl) units.push_back(phase | (sl << 2));
+            };
+            for (int k = 0; k <= G; ++k) { emit(0, k); emit(2, k - 1); emit(1, k); }
+            h->fused_nslab = nslab;
+            h->fused_nunits = (int)units.size();
+            h->fused_gs = gs;
+            if ((rc = upload(h, units, &h->fused_units))) return rc;
+            CU(cudaMalloc(&h->fused_ctr, sizeof(unsigned int) * (size_t)(1 + 2 * nslab)));
+            h->owned.push_back(h->fused_ctr);
+            h->fused_fft = true;
+        }
     }
     return DGPE_OK;
 }
 
-extern "C" dgpe_handle* dgpe_create(int nx, int ny, int nz, double dx, double dy, double dz, double dt,
-                                    double gamma, double nu, double lambda, double g, double gdd, int mode)
+static thread_local int g_err_code = DGPE_OK;
+
+extern "C" int dgpe_last_error_code(void) { return g_err_code; }
+
+extern "C" dgpe_handle* dgpe_create_ex(int nx, int ny, int nz, double dx, double dy, double dz, double dt,
+                                       double gamma, double nu, double lambda, double g, double gdd, int mode,
+                                       const dgpe_options* opt)
 {
     g_err[0] = 0;
+    g_err_code = DGPE_OK;
+    auto bad = [](int code) -> dgpe_handle* { g_err_code = code; return nullptr; };
     const int ns[3] = {nx, ny, nz};
     for (int a = 0; a < 3; ++a) {
-        if (ns[a] < 4) { fail(DGPE_ERR_ARG, "grid size %d < 4", ns[a]); return nullptr; }
-        if (!smooth2357(ns[a])) { fail(DGPE_ERR_ARG, "grid size %d is not of the form 2^a 3^b 5^c 7^d 11^e 13^f", ns[a]); return nullptr; }
-        if (ns[a] > DGPE_MAX_N) { fail(DGPE_ERR_UNSUPPORTED, "grid size %d > %d", ns[a], DGPE_MAX_N); return nullptr; }
+        if (ns[a] < 4) return bad(fail(DGPE_ERR_ARG, "grid size %d < 4", ns[a]));
+        if (!smooth2357(ns[a])) return bad(fail(DGPE_ERR_ARG, "grid size %d is not of the form 2^a 3^b 5^c 7^d 11^e 13^f", ns[a]));
+        if (ns[a] > DGPE_MAX_N) return bad(fail(DGPE_ERR_UNSUPPORTED, "grid size %d > %d", ns[a], DGPE_MAX_N));
     }
-    if (nz % 2) { fail(DGPE_ERR_ARG, "nz = %d must be even", nz); return nullptr; }
+    if (nz % 2) return bad(fail(DGPE_ERR_ARG, "nz = %d must be even", nz));
     if (!(dx > 0.0) || !(dy > 0.0) || !(dz > 0.0) || !(dt > 0.0) || !std::isfinite(dx) || !std::isfinite(dy) ||
-        !std::isfinite(dz) || !std::isfinite(dt)) {
-        fail(DGPE_ERR_ARG, "dx, dy, dz, dt must be positive and finite");
-        return nullptr;
-    }
-    if (mode != DGPE_IMAG && mode != DGPE_REAL && mode != DGPE_IMAG_RPSI) {
-        fail(DGPE_ERR_ARG, "mode %d is none of DGPE_IMAG, DGPE_REAL, DGPE_IMAG_RPSI", mode);
-        return nullptr;
-    }
+        !std::isfinite(dz) || !std::isfinite(dt))
+        return bad(fail(DGPE_ERR_ARG, "dx, dy, dz, dt must be positive and finite"));
+    if (mode != DGPE_IMAG && mode != DGPE_REAL && mode != DGPE_IMAG_RPSI)
+        return bad(fail(DGPE_ERR_ARG, "mode %d is none of DGPE_IMAG, DGPE_REAL, DGPE_IMAG_RPSI", mode));
     dgpe_handle* h = new (std::nothrow) dgpe_handle();
-    if (!h) { fail(DGPE_ERR_NOMEM, "host allocation failed"); return nullptr; }
+    if (!h) return bad(fail(DGPE_ERR_NOMEM, "host allocation failed"));
+    if (opt) h->opt = *opt;
+    else { int* f = reinterpret_cast<int*>(&h->opt); for (size_t i = 0; i < sizeof(dgpe_options) / sizeof(int); ++i) f[i] = -1; }
     h->nx = nx; h->ny = ny; h->nz = nz; h->nzh = nz / 2 + 1;
     h->rpsi = mode == DGPE_IMAG_RPSI;
     h->mode = h->rpsi ? DGPE_IMAG : mode;
@@ -478,21 +487,28 @@ extern "C" dgpe_handle* dgpe_create(int nx, int ny, int nz, double dx, double dy
     h->dx = dx; h->dy = dy; h->dz = dz; h->dt = dt;
     h->gamma = gamma; h->nu = nu; h->lambda = lambda; h->g = g; h->gdd = gdd;
     h->N = (long long)nx * ny * nz;
-    if (init_handle(h) != DGPE_OK) {
+    const int rc = init_handle(h);
+    if (rc != DGPE_OK) {
         char keep[sizeof(g_err)];
         std::memcpy(keep, g_err, sizeof(keep));
         dgpe_destroy(h);
         std::memcpy(g_err, keep, sizeof(keep));
-        return nullptr;
+        return bad(rc);
     }
     return h;
+}
+
+extern "C" dgpe_handle* dgpe_create(int nx, int ny, int nz, double dx, double dy, double dz, double dt,
+                                    double gamma, double nu, double lambda, double g, double gdd, int mode)
+{
+    return dgpe_create_ex(nx, ny, nz, dx, dy, dz, dt, gamma, nu, lambda, g, gdd, mode, nullptr);
 }
 
 extern "C" void dgpe_destroy(dgpe_handle* h)
 {
     if (!h) return;
     cudaStreamSynchronize(h->stream);
-    if (h->step_exec) cudaGraphExecDestroy(h->step_exec);
+    for (auto& e : h->step_execs) cudaGraphExecDestroy(e.second);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     for (void* p : h->owned) cudaFree(p);
     if (h->h_out) cudaFreeHost(h->h_out);
@@ -517,6 +533,16 @@ extern "C" int dgpe_synchronize(dgpe_handle* h)
 // ------------------------------------------------------------------------------------------------
 // launches
 // ------------------------------------------------------------------------------------------------
+// every call must run with the handle's device current (kernels, tensor maps and pointers belong to it)
+static int check_device(const dgpe_handle* h)
+{
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev != h->device)
+        return fail(DGPE_ERR_ARG, "the handle lives on CUDA device %d but device %d is current", h->device, dev);
+    return DGPE_OK;
+}
+
 static int check_launch(const char* what)
 {
     cudaError_t e = cudaGetLastError();
@@ -681,8 +707,11 @@ static int launch_k1(dgpe_handle* h, const cplx* psi)
 {
     if (h->zfast) return launch_z_r2c(h, psi);
     const int nlines = h->nx * h->ny, M = h->nz / 2;
-    k_dens_r2c<<<(nlines + 7) / 8, threads_for(h->plan_zh.nbf), sizeof(cplx) * TILE_COLS * (size_t)M, h->stream>>>(
-        psi, h->spec, nlines, h->nz, h->plan_zh, h->tw_split, h->scal);
+    const int thr = threads_for(h->plan_zh.nbf);
+    const size_t sm = sizeof(cplx) * TILE_COLS * (size_t)M;
+    int rcs = kernel_setup((const void*)k_dens_r2c, thr, sm, nullptr);
+    if (rcs) return rcs;
+    k_dens_r2c<<<(nlines + 7) / 8, thr, sm, h->stream>>>(psi, h->spec, nlines, h->nz, h->plan_zh, h->tw_split, h->scal);
     return check_launch("k_dens_r2c");
 }
 
@@ -862,12 +891,23 @@ static int launch_fft_y(dgpe_handle* h, bool inverse)
     dim3 gy((nzh + 7) / 8, nx);
     const int ty = threads_for(h->plan_y.nbf);
     const size_t smy = sizeof(cplx) * TILE_COLS * (size_t)ny;
+    int rcs;
     if (inverse) {
-        if (ty <= 512) k_fft_lines<true, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
-        else k_fft_lines<true, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+        if (ty <= 512) {
+            if ((rcs = kernel_setup((const void*)k_fft_lines<true, 512>, ty, smy, nullptr))) return rcs;
+            k_fft_lines<true, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+        } else {
+            if ((rcs = kernel_setup((const void*)k_fft_lines<true, 1024>, ty, smy, nullptr))) return rcs;
+            k_fft_lines<true, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+        }
     } else {
-        if (ty <= 512) k_fft_lines<false, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
-        else k_fft_lines<false, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+        if (ty <= 512) {
+            if ((rcs = kernel_setup((const void*)k_fft_lines<false, 512>, ty, smy, nullptr))) return rcs;
+            k_fft_lines<false, 512><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+        } else {
+            if ((rcs = kernel_setup((const void*)k_fft_lines<false, 1024>, ty, smy, nullptr))) return rcs;
+            k_fft_lines<false, 1024><<<gy, ty, smy, h->stream>>>(h->spec, my, h->plan_y);
+        }
     }
     return check_launch("k_fft_lines<y>");
 }
@@ -885,13 +925,61 @@ static int launch_fft_x_udd(dgpe_handle* h)
     }
     const int tx = threads_for(h->plan_x.nbf);
     const size_t smx = sizeof(cplx) * TILE_COLS * (size_t)nx;
-    if (tx <= 512)
+    int rcs;
+    if (tx <= 512) {
+        if ((rcs = kernel_setup((const void*)k_fft_x_udd<512>, tx, smx, nullptr))) return rcs;
         k_fft_x_udd<512><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
                                                                      1.0 / (double)h->N);
-    else
+    } else {
+        if ((rcs = kernel_setup((const void*)k_fft_x_udd<1024>, tx, smx, nullptr))) return rcs;
         k_fft_x_udd<1024><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
                                                                       1.0 / (double)h->N);
+    }
     return check_launch("k_fft_x_udd");
+}
+
+// ---- K2 + K3 + K4 as one launch over L2-resident kz slabs (xyfft_fused.cuh) ----
+#define DGPE_FUSED_SIZES(X) X(64) X(128) X(192) X(256) X(320) X(384) X(480) X(512)
+
+static bool fused_fft_supported(int nx, int ny)
+{
+    if (nx != ny) return false;
+    switch (nx) {
+#define X(NN) case NN:
+        DGPE_FUSED_SIZES(X)
+#undef X
+        return true;
+        default: return false;
+    }
+}
+
+template <int N>
+static int launch_fft_fused_n(dgpe_handle* h)
+{
+    auto kern = k_fft_yxy<N>;
+    const size_t smem = (size_t)N * TILE_COLS * sizeof(cplx);
+    int ctas_per_sm = 0;
+    int rc = kernel_setup((const void*)kern, xy_threads<N>(), smem, &ctas_per_sm);
+    if (rc) return rc;
+    CU(cudaMemsetAsync(h->fused_ctr, 0, sizeof(unsigned int) * (size_t)(1 + 2 * h->fused_nslab), h->stream));
+    const int nitems = h->fused_nunits * N;      // one CTA per tile; the CTAs claim their tiles in queue order
+    FusedWalk W;
+    W.ny = h->ny; W.nzh = h->nzh; W.nslab = h->fused_nslab; W.nunits = h->fused_nunits;
+    W.units = h->fused_units; W.head = h->fused_ctr; W.done = h->fused_ctr + 1;
+    W.pf_items = (h->prefetch & PF_FFT_Y) ? h->pf_mult * ctas_per_sm * h->num_sms : 0;
+    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 2.0 * 3.14159265358979323846264338327950288 / ((double)h->nx * h->dx), 1.0 / (double)h->N, 0};
+    kern<<<nitems, xy_threads<N>(), smem, h->stream>>>(h->spec, W, h->tw_y, U);
+    return check_launch("k_fft_yxy");
+}
+
+static int launch_fft_fused(dgpe_handle* h)
+{
+    switch (h->nx) {
+#define X(NN) case NN: return launch_fft_fused_n<NN>(h);
+        DGPE_FUSED_SIZES(X)
+#undef X
+        default: return fail(DGPE_ERR_UNSUPPORTED, "no fused FFT kernel for nx = ny = %d", h->nx);
+    }
 }
 
 // K1..K4: spec <- Udd~(k)/N * FFT(s2 |psi|^2), transformed back along x and y
@@ -899,6 +987,7 @@ static int launch_dipolar_spectrum(dgpe_handle* h, const cplx* psi)
 {
     int rc;
     if ((rc = launch_k1(h, psi))) return rc;
+    if (h->fused_fft) return launch_fft_fused(h);
     if ((rc = launch_fft_y(h, false))) return rc;
     if ((rc = launch_fft_x_udd(h))) return rc;
     return launch_fft_y(h, true);
@@ -916,12 +1005,20 @@ static int launch_c2r(dgpe_handle* h, cplx* psi, int kmode, double* out)
     A.scal = h->scal; A.partials = h->partials; A.ticket = h->ticket; A.out = out;
     const int grid = (nlines + 7) / 8, thr = threads_for(h->plan_zh.nbf);
     const size_t sm = sizeof(cplx) * TILE_COLS * (size_t)(M + 1);
+    auto go = [&](auto kern, auto* p) -> int {
+        int rcs = kernel_setup((const void*)kern, thr, sm, nullptr);
+        if (rcs) return rcs;
+        kern<<<grid, thr, sm, h->stream>>>(p, h->spec, h->plan_zh, h->tw_split, A);
+        return DGPE_OK;
+    };
+    int rcs;
     switch (kmode) {
-        case 0: k_c2r_nonlin<0><<<grid, thr, sm, h->stream>>>(psi, h->spec, h->plan_zh, h->tw_split, A); break;
-        case 1: k_c2r_nonlin<1><<<grid, thr, sm, h->stream>>>(psi, h->spec, h->plan_zh, h->tw_split, A); break;
-        case 2: k_c2r_nonlin<2><<<grid, thr, sm, h->stream>>>(psi, h->spec, h->plan_zh, h->tw_split, A); break;
-        default: k_c2r_nonlin<3><<<grid, thr, sm, h->stream>>>(psi, h->spec, h->plan_zh, h->tw_split, A); break;
+        case 0: rcs = go(k_c2r_nonlin<0, cplx>, psi); break;
+        case 1: rcs = go(k_c2r_nonlin<1, cplx>, psi); break;
+        case 2: rcs = h->rpsi ? go(k_c2r_nonlin<2, double>, (double*)psi) : go(k_c2r_nonlin<2, cplx>, psi); break;
+        default: rcs = go(k_c2r_nonlin<3, cplx>, psi); break;
     }
+    if (rcs) return rcs;
     return check_launch("k_c2r_nonlin");
 }
 
@@ -1043,16 +1140,23 @@ static int launch_sweep_t(dgpe_handle* h, cplx* psi, int axis, bool fold)
             return S.consttab ? launch_sweep_xy<CT, 16, true, 512, 1>(h, psi, m, grid, thr, T, F, S)
                               : launch_sweep_xy<CT, 16, false, 512, 1>(h, psi, m, grid, thr, T, F, S);
     }
+    int rcs;
     if (axis == 0) {
         LineMap m{nx, ny * nz, 0, 1, (long long)ny * nz};
-        k_sweep<CT, false><<<(ny * nz + 7) / 8, thr, sweep_smem(nx, S.G, false), h->stream>>>(psi, m, T, F);
+        const size_t sm = sweep_smem(nx, S.G, false);
+        if ((rcs = kernel_setup((const void*)k_sweep<CT, false>, thr, sm, nullptr))) return rcs;
+        k_sweep<CT, false><<<(ny * nz + 7) / 8, thr, sm, h->stream>>>(psi, m, T, F);
     } else if (axis == 1) {
         LineMap m{ny, nz, (long long)ny * nz, 1, nz};
         dim3 grid((nz + 7) / 8, nx);
-        k_sweep<CT, false><<<grid, thr, sweep_smem(ny, S.G, false), h->stream>>>(psi, m, T, F);
+        const size_t sm = sweep_smem(ny, S.G, false);
+        if ((rcs = kernel_setup((const void*)k_sweep<CT, false>, thr, sm, nullptr))) return rcs;
+        k_sweep<CT, false><<<grid, thr, sm, h->stream>>>(psi, m, T, F);
     } else {
         LineMap m{nz, nx * ny, 0, nz, 1};
-        k_sweep<CT, true><<<(nx * ny + 7) / 8, thr, sweep_smem(nz, S.G, true), h->stream>>>(psi, m, T, F);
+        const size_t sm = sweep_smem(nz, S.G, true);
+        if ((rcs = kernel_setup((const void*)k_sweep<CT, true>, thr, sm, nullptr))) return rcs;
+        k_sweep<CT, true><<<(nx * ny + 7) / 8, thr, sm, h->stream>>>(psi, m, T, F);
     }
     return check_launch("k_sweep");
 }
@@ -1069,52 +1173,81 @@ static int set_scal(dgpe_handle* h, int clear_bad)
     return check_launch("k_set_scal");
 }
 
-// One step = 8 kernels in the order of the method (K1..K5, sweeps x, y, z), or 7 when the z-line
-// kernels are available: the z sweep then runs fused into K5 and the sweeps go z, x, y (the three 1-D
-// Cayley operators commute: R#26), with the norm folded into the last sweep either way.
-// `mark` is called after each launch with the kernel index.
-static const char* const KERNEL_NAMES8[8] = {"K1 dens_r2c(z)", "K2 fft_y fwd", "K3 fft_x*Udd*ifft_x", "K4 fft_y inv",
-                                             "K5 c2r(z)+nonlinear", "K6 sweep_x", "K7 sweep_y", "K8 sweep_z(+norm)"};
-static const char* const KERNEL_NAMES7[7] = {"K1 dens_r2c(z)", "K2 fft_y fwd", "K3 fft_x*Udd*ifft_x", "K4 fft_y inv",
-                                             "K5+K8 c2r(z)+nonlinear+sweep_z", "K6 sweep_x", "K7 sweep_y(+norm)"};
+// One step = 8 kernels in the order of the method (K1..K5, sweeps x, y, z); 7 when the z-line kernels are
+// available: the z sweep then runs fused into K5 and the sweeps go z, x, y (the three 1-D Cayley operators
+// commute: R#26); 5 when K2, K3, K4 also run as the one L2-resident slab kernel.  The norm is folded into the
+// last sweep either way.  `mark` is called after each launch with the kernel index.
+struct StepKernel { const char* name; double bytes; };
+
+// the kernels of one step AS BUILT with their algorithmic bytes (each array read once and written once per pass)
+static std::vector<StepKernel> step_kernels(const dgpe_handle* h)
+{
+    const double S = 16.0 * (double)h->nx * h->ny * h->nzh;
+    const double N = (h->rpsi ? 0.5 : 1.0) * (double)h->N;      // in units of 16 bytes of psi
+    std::vector<StepKernel> k;
+    k.push_back({"K1 dens_r2c(z)", 16.0 * N + S});
+    if (h->fused_fft) {
+        k.push_back({"K2+K3+K4 fft_y.fft_x*Udd*ifft_x.ifft_y (L2-resident slabs)", 2.0 * S});
+    } else {
+        k.push_back({"K2 fft_y fwd", 2.0 * S});
+        k.push_back({"K3 fft_x*Udd*ifft_x", 2.0 * S});
+        k.push_back({"K4 fft_y inv", 2.0 * S});
+    }
+    if (h->zfast) {
+        k.push_back({"K5+K8 c2r(z)+nonlinear+sweep_z", S + 32.0 * N});     // the fused z sweep adds no traffic
+        k.push_back({"K6 sweep_x", 32.0 * N});
+        k.push_back({"K7 sweep_y(+norm)", 32.0 * N});
+    } else {
+        k.push_back({"K5 c2r(z)+nonlinear", S + 32.0 * N});
+        k.push_back({"K6 sweep_x", 32.0 * N});
+        k.push_back({"K7 sweep_y", 32.0 * N});
+        k.push_back({"K8 sweep_z(+norm)", 32.0 * N});
+    }
+    return k;
+}
 
 template <typename Mark>
 static int one_step(dgpe_handle* h, cplx* psi, Mark mark)
 {
     const bool imag = h->mode == DGPE_IMAG;
-    int rc;
+    int rc, k = 0;
     if ((rc = launch_k1(h, psi))) return rc;
-    mark(0);
-    if ((rc = launch_fft_y(h, false))) return rc;
-    mark(1);
-    if ((rc = launch_fft_x_udd(h))) return rc;
-    mark(2);
-    if ((rc = launch_fft_y(h, true))) return rc;
-    mark(3);
+    mark(k++);
+    if (h->fused_fft) {
+        if ((rc = launch_fft_fused(h))) return rc;
+        mark(k++);
+    } else {
+        if ((rc = launch_fft_y(h, false))) return rc;
+        mark(k++);
+        if ((rc = launch_fft_x_udd(h))) return rc;
+        mark(k++);
+        if ((rc = launch_fft_y(h, true))) return rc;
+        mark(k++);
+    }
     if (h->zfast) {
         if ((rc = launch_z_main(h, psi, 1, nullptr))) return rc;
-        mark(4);
+        mark(k++);
         if ((rc = launch_sweep(h, psi, 0, false))) return rc;
-        mark(5);
+        mark(k++);
         if ((rc = launch_sweep(h, psi, 1, imag))) return rc;
-        mark(6);
+        mark(k++);
         return DGPE_OK;
     }
     if ((rc = launch_c2r(h, psi, imag ? 0 : 1, nullptr))) return rc;
-    mark(4);
+    mark(k++);
     if ((rc = launch_sweep(h, psi, 0, false))) return rc;
-    mark(5);
+    mark(k++);
     if ((rc = launch_sweep(h, psi, 1, false))) return rc;
-    mark(6);
+    mark(k++);
     if ((rc = launch_sweep(h, psi, 2, imag))) return rc;
-    mark(7);
+    mark(k++);
     return DGPE_OK;
 }
 
 static int finish_steps(dgpe_handle* h, cplx* psi)
 {
     int rc;
-    k_scale<<<148 * 8, 256, 0, h->stream>>>(psi, h->rpsi ? h->N / 2 : h->N, h->scal);
+    k_scale<<<h->num_sms * 8, 256, 0, h->stream>>>(psi, h->rpsi ? h->N / 2 : h->N, h->scal);
     if ((rc = check_launch("k_scale"))) return rc;
     CU(cudaMemcpyAsync(h->h_out, h->scal, sizeof(double) * SC_COUNT, cudaMemcpyDeviceToHost, h->stream));
     return set_scal(h, 0);
@@ -1138,8 +1271,14 @@ static int run_steps(dgpe_handle* h, cplx* psi, int nsteps)
         s = 1;
     }
     if (h->use_graph && nsteps - s >= 2) {
-        if (!h->step_exec || h->step_exec_psi != psi) {
-            if (h->step_exec) { cudaGraphExecDestroy(h->step_exec); h->step_exec = nullptr; }
+        cudaGraphExec_t exec = nullptr;
+        for (size_t i = 0; i < h->step_execs.size(); ++i)
+            if (h->step_execs[i].first == psi) {
+                std::rotate(h->step_execs.begin(), h->step_execs.begin() + i, h->step_execs.begin() + i + 1);
+                exec = h->step_execs[0].second;
+                break;
+            }
+        if (!exec) {
             if (!h->cap_stream) CU(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
             cudaStream_t user = h->stream;
             h->stream = h->cap_stream;
@@ -1153,12 +1292,16 @@ static int run_steps(dgpe_handle* h, cplx* psi, int nsteps)
                 cudaGetLastError();
                 return fail(DGPE_ERR_CUDA, "capturing the step graph failed: %s", cudaGetErrorString(e2));
             }
-            e = cudaGraphInstantiate(&h->step_exec, graph, 0);
+            e = cudaGraphInstantiate(&exec, graph, 0);
             cudaGraphDestroy(graph);
-            if (e != cudaSuccess) { h->step_exec = nullptr; return fail(DGPE_ERR_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e)); }
-            h->step_exec_psi = psi;
+            if (e != cudaSuccess) return fail(DGPE_ERR_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e));
+            if (h->step_execs.size() >= 4) {
+                cudaGraphExecDestroy(h->step_execs.back().second);
+                h->step_execs.pop_back();
+            }
+            h->step_execs.insert(h->step_execs.begin(), std::make_pair(psi, exec));
         }
-        for (; s < nsteps; ++s) CU(cudaGraphLaunch(h->step_exec, h->stream));
+        for (; s < nsteps; ++s) CU(cudaGraphLaunch(exec, h->stream));
         return DGPE_OK;
     }
     for (; s < nsteps; ++s)
@@ -1169,6 +1312,7 @@ static int run_steps(dgpe_handle* h, cplx* psi, int nsteps)
 extern "C" int dgpe_step(dgpe_handle* h, void* psi_, int nsteps)
 {
     if (!h || !psi_) return fail(DGPE_ERR_ARG, "NULL handle or psi");
+    { int rcd = check_device(h); if (rcd) return rcd; }
     if (nsteps < 0) return fail(DGPE_ERR_ARG, "nsteps = %d < 0", nsteps);
     if (nsteps == 0) return DGPE_OK;
     cplx* psi = (cplx*)psi_;
@@ -1186,6 +1330,7 @@ extern "C" int dgpe_step(dgpe_handle* h, void* psi_, int nsteps)
 extern "C" int dgpe_step_host(dgpe_handle* h, void* psi_host, int nsteps)
 {
     if (!h || !psi_host) return fail(DGPE_ERR_ARG, "NULL handle or psi");
+    { int rcd = check_device(h); if (rcd) return rcd; }
     if (nsteps < 0) return fail(DGPE_ERR_ARG, "nsteps = %d < 0", nsteps);
     const size_t bytes = (h->rpsi ? sizeof(double) : sizeof(cplx)) * (size_t)h->N;
     if (!h->psi_stage) {
@@ -1211,6 +1356,7 @@ extern "C" int dgpe_step_host(dgpe_handle* h, void* psi_host, int nsteps)
 extern "C" int dgpe_step_profile(dgpe_handle* h, void* psi_, int nsteps, double* ms)
 {
     if (!h || !psi_ || !ms) return fail(DGPE_ERR_ARG, "NULL argument");
+    { int rcd = check_device(h); if (rcd) return rcd; }
     if (nsteps < 1) return fail(DGPE_ERR_ARG, "nsteps = %d < 1", nsteps);
     const int NK = dgpe_launches_per_step(h);
     const size_t need = (size_t)nsteps * (NK + 1);
@@ -1245,23 +1391,14 @@ extern "C" int dgpe_step_profile(dgpe_handle* h, void* psi_, int nsteps, double*
 extern "C" const char* dgpe_kernel_name(const dgpe_handle* h, int k)
 {
     if (!h || k < 0 || k >= dgpe_launches_per_step(h)) return "";
-    return h->zfast ? KERNEL_NAMES7[k] : KERNEL_NAMES8[k];
+    return step_kernels(h)[k].name;
 }
 
 // algorithmic bytes of kernel k AS BUILT: each array read once and written once per pass
 extern "C" double dgpe_kernel_bytes(const dgpe_handle* h, int k)
 {
-    if (!h) return 0.0;
-    const double S = 16.0 * (double)h->nx * h->ny * h->nzh;
-    const double N = (h->rpsi ? 0.5 : 1.0) * (double)h->N;      // in units of 16 bytes of psi
-    switch (k) {
-        case 0: return 16.0 * N + S;       // read psi, write half-spectrum
-        case 1: case 2: case 3: return 2.0 * S;
-        case 4: return S + 32.0 * N;       // read spectrum, read + write psi (the fused z sweep adds no traffic)
-        case 5: case 6: return 32.0 * N;
-        case 7: return h->zfast ? 0.0 : 32.0 * N;
-        default: return 0.0;
-    }
+    if (!h || k < 0 || k >= dgpe_launches_per_step(h)) return 0.0;
+    return step_kernels(h)[k].bytes;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1270,6 +1407,7 @@ extern "C" double dgpe_kernel_bytes(const dgpe_handle* h, int k)
 extern "C" int dgpe_dipolar(dgpe_handle* h, const void* psi, void* phi)
 {
     if (!h || !psi || !phi) return fail(DGPE_ERR_ARG, "NULL argument");
+    { int rcd = check_device(h); if (rcd) return rcd; }
     int rc;
     if ((rc = launch_dipolar_spectrum(h, (const cplx*)psi))) return rc;
     return launch_c2r(h, const_cast<cplx*>((const cplx*)psi), 3, (double*)phi);
@@ -1278,6 +1416,7 @@ extern "C" int dgpe_dipolar(dgpe_handle* h, const void* psi, void* phi)
 extern "C" int dgpe_nonlinear(dgpe_handle* h, void* psi)
 {
     if (!h || !psi) return fail(DGPE_ERR_ARG, "NULL argument");
+    { int rcd = check_device(h); if (rcd) return rcd; }
     int rc;
     if ((rc = launch_dipolar_spectrum(h, (const cplx*)psi))) return rc;
     return launch_c2r(h, (cplx*)psi, h->mode == DGPE_IMAG ? 0 : 1, nullptr);
@@ -1286,6 +1425,7 @@ extern "C" int dgpe_nonlinear(dgpe_handle* h, void* psi)
 extern "C" int dgpe_sweep(dgpe_handle* h, void* psi, int axis)
 {
     if (!h || !psi) return fail(DGPE_ERR_ARG, "NULL argument");
+    { int rcd = check_device(h); if (rcd) return rcd; }
     if (axis < 0 || axis > 2) return fail(DGPE_ERR_ARG, "axis %d not in 0..2", axis);
     return launch_sweep(h, (cplx*)psi, axis, false);
 }
@@ -1309,44 +1449,11 @@ static int fetch(dgpe_handle* h, int count)
     return DGPE_OK;
 }
 
-// Observables of a real-valued psi (DGPE_IMAG_RPSI; not on the timed path): psi is copied into a complex
-// array the handle owns and the handle behaves as a complex-psi one until the view is dropped.
-struct ComplexView {
-    dgpe_handle* h;
-    const void* psi;
-    bool widened = false;
-    int rc = DGPE_OK;
-    ComplexView(dgpe_handle* h_, const void* psi_) : h(h_), psi(psi_)
-    {
-        if (!h->rpsi) return;
-        if (!h->psi_wide) {
-            if (cudaMalloc(&h->psi_wide, sizeof(cplx) * (size_t)h->N) != cudaSuccess) {
-                cudaGetLastError();
-                rc = fail(DGPE_ERR_NOMEM, "no device memory for the complex copy of psi (%lld bytes)", 16LL * h->N);
-                return;
-            }
-            h->owned.push_back(h->psi_wide);
-        }
-        k_widen<<<148 * 8, 256, 0, h->stream>>>((const double*)psi_, h->psi_wide, h->N);
-        if ((rc = check_launch("k_widen"))) return;
-        psi = h->psi_wide;
-        h->rpsi = false;
-        h->nzc = h->nz;
-        widened = true;
-    }
-    ~ComplexView()
-    {
-        if (widened) { h->rpsi = true; h->nzc = h->nz / 2; }
-    }
-};
-
-static int moments(dgpe_handle* h, const void* psi_)
+static int moments(dgpe_handle* h, const void* psi)
 {
-    ComplexView view(h, psi_);
-    if (view.rc) return view.rc;
-    const void* psi = view.psi;
-    const int grid = std::min(h->nx * h->ny, 148 * 8);
-    k_moments<<<grid, 256, 0, h->stream>>>((const cplx*)psi, obs_args(h, h->d_out));
+    const int grid = std::min(h->nx * h->ny, h->num_sms * 8);
+    if (h->rpsi) k_moments<double><<<grid, 256, 0, h->stream>>>((const double*)psi, obs_args(h, h->d_out));
+    else k_moments<cplx><<<grid, 256, 0, h->stream>>>((const cplx*)psi, obs_args(h, h->d_out));
     int rc = check_launch("k_moments");
     if (rc) return rc;
     return fetch(h, 4);
@@ -1355,6 +1462,7 @@ static int moments(dgpe_handle* h, const void* psi_)
 extern "C" int dgpe_norm(dgpe_handle* h, const void* psi, double* norm)
 {
     if (!h || !psi || !norm) return fail(DGPE_ERR_ARG, "NULL argument");
+    { int rcd = check_device(h); if (rcd) return rcd; }
     int rc = moments(h, psi);
     if (rc) return rc;
     *norm = h->h_out[0] * h->dx * h->dy * h->dz;
@@ -1364,6 +1472,7 @@ extern "C" int dgpe_norm(dgpe_handle* h, const void* psi, double* norm)
 extern "C" int dgpe_rms(dgpe_handle* h, const void* psi, double rms[4])
 {
     if (!h || !psi || !rms) return fail(DGPE_ERR_ARG, "NULL argument");
+    { int rcd = check_device(h); if (rcd) return rcd; }
     int rc = moments(h, psi);
     if (rc) return rc;
     const double s = h->h_out[0];
@@ -1377,14 +1486,14 @@ extern "C" int dgpe_rms(dgpe_handle* h, const void* psi, double rms[4])
 extern "C" int dgpe_energy_terms(dgpe_handle* h, const void* psi_, double out[4])
 {
     if (!h || !psi_ || !out) return fail(DGPE_ERR_ARG, "NULL argument");
-    ComplexView view(h, psi_);
-    if (view.rc) return view.rc;
-    const void* psi = view.psi;
+    const void* psi = psi_;      // complex, or plain doubles in DGPE_IMAG_RPSI: every kernel below takes either
     int rc;
+    if ((rc = check_device(h))) return rc;
     if ((rc = launch_dipolar_spectrum(h, (const cplx*)psi))) return rc;
     if ((rc = launch_c2r(h, const_cast<cplx*>((const cplx*)psi), 2, h->d_out))) return rc;
-    const int grid = std::min(h->nx * h->ny, 148 * 8);
-    k_kinetic<<<grid, 256, 0, h->stream>>>((const cplx*)psi, obs_args(h, h->d_out + 4));
+    const int grid = std::min(h->nx * h->ny, h->num_sms * 8);
+    if (h->rpsi) k_kinetic<double><<<grid, 256, 0, h->stream>>>((const double*)psi, obs_args(h, h->d_out + 4));
+    else k_kinetic<cplx><<<grid, 256, 0, h->stream>>>((const cplx*)psi, obs_args(h, h->d_out + 4));
     if ((rc = check_launch("k_kinetic"))) return rc;
     if ((rc = fetch(h, 8))) return rc;
     const double sV = h->h_out[0], sg = h->h_out[1], sdd = h->h_out[2], s = h->h_out[3];
@@ -1427,5 +1536,5 @@ extern "C" double dgpe_bytes_per_step(const dgpe_handle* h)
 
 extern "C" int dgpe_launches_per_step(const dgpe_handle* h)
 {
-    return (h && h->zfast) ? 7 : 8;
+    return h ? (int)step_kernels(h).size() : 0;
 }

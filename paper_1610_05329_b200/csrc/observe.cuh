@@ -13,15 +13,10 @@ struct ObsArgs {
     double* out;
 };
 
-// complex copy of a real-valued psi (DGPE_IMAG_RPSI observables)
-__global__ void k_widen(const double* __restrict__ src, cplx* __restrict__ dst, long long N)
-{
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < N; p += stride) dst[p] = mk(src[p], 0.0);
-}
-
 // out[0..3] = sum n, sum x^2 n, sum y^2 n, sum z^2 n      (n = |psi|^2)
-__global__ void k_moments(const cplx* __restrict__ psi, ObsArgs A)
+// DT = cplx, or double for a real-valued psi (DGPE_IMAG_RPSI)
+template <typename DT>
+__global__ void k_moments(const DT* __restrict__ psi, ObsArgs A)
 {
     __shared__ double red[32 * 4];
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
@@ -29,7 +24,7 @@ __global__ void k_moments(const cplx* __restrict__ psi, ObsArgs A)
     for (int line = blockIdx.x; line < nlines; line += gridDim.x) {
         const int i = line / A.ny, j = line - i * A.ny;
         const double xx = __ldg(&A.x2[i]), yy = __ldg(&A.y2[j]);
-        const cplx* p = psi + (long long)line * A.nz;
+        const DT* p = psi + (long long)line * A.nz;
         for (int k = threadIdx.x; k < A.nz; k += blockDim.x) {
             const double n = cabs2(p[k]);
             acc[0] += n;
@@ -47,7 +42,8 @@ __global__ void k_moments(const cplx* __restrict__ psi, ObsArgs A)
 
 // out[0..2] = sum over links along x, y, z of |psi_{j+1} - psi_j|^2, links j = -1..n-1 with the
 // ghost nodes psi_{-1} = psi_n = 0   (R#16)
-__global__ void k_kinetic(const cplx* __restrict__ psi, ObsArgs A)
+template <typename DT>
+__global__ void k_kinetic(const DT* __restrict__ psi, ObsArgs A)
 {
     __shared__ double red[32 * 3];
     double acc[3] = {0.0, 0.0, 0.0};
@@ -55,13 +51,13 @@ __global__ void k_kinetic(const cplx* __restrict__ psi, ObsArgs A)
     const long long sy = A.nz, sx = (long long)A.ny * A.nz;
     for (int line = blockIdx.x; line < nlines; line += gridDim.x) {
         const int i = line / A.ny, j = line - i * A.ny;
-        const cplx* p = psi + (long long)line * A.nz;
+        const DT* p = psi + (long long)line * A.nz;
         for (int k = threadIdx.x; k < A.nz; k += blockDim.x) {
-            const cplx here = p[k];
-            const cplx zero = mk(0.0, 0.0);
-            const cplx px = (i + 1 < A.nx) ? p[k + sx] : zero;
-            const cplx py = (j + 1 < A.ny) ? p[k + sy] : zero;
-            const cplx pz = (k + 1 < A.nz) ? p[k + 1] : zero;
+            const DT here = p[k];
+            const DT zero = DT();
+            const DT px = (i + 1 < A.nx) ? p[k + sx] : zero;
+            const DT py = (j + 1 < A.ny) ? p[k + sy] : zero;
+            const DT pz = (k + 1 < A.nz) ? p[k + 1] : zero;
             acc[0] += cabs2(csub(px, here));
             acc[1] += cabs2(csub(py, here));
             acc[2] += cabs2(csub(pz, here));

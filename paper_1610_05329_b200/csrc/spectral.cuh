@@ -141,8 +141,9 @@ struct NonlinArgs {
     double* out;               // MODE 2: 4 totals;  MODE 3: phi_out
 };
 
-template <int MODE>
-__global__ void __launch_bounds__(512, 1) k_c2r_nonlin(cplx* __restrict__ psi, const cplx* __restrict__ spec, FftPlan P,
+// DT = element type of psi: cplx, or double for the observables (MODE 2) of a real-valued psi (DGPE_IMAG_RPSI)
+template <int MODE, typename DT>
+__global__ void __launch_bounds__(512, 1) k_c2r_nonlin(DT* __restrict__ psi, const cplx* __restrict__ spec, FftPlan P,
                              const cplx* __restrict__ tws, NonlinArgs A)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -185,7 +186,7 @@ __global__ void __launch_bounds__(512, 1) k_c2r_nonlin(cplx* __restrict__ psi, c
         const int i = line / A.ny, j = line - i * A.ny;
         const double vxy = __ldg(&A.vx[i]) + __ldg(&A.vy[j]);
         const double s2 = A.scal[SC_S2], s1 = A.scal[SC_S1];
-        cplx* p = psi + (long long)line * nz;
+        DT* p = psi + (long long)line * nz;
         for (int m = b; m < M; m += nb) {
             const cplx phi = sm[m * TILE_COLS + c];
             if (MODE == 3) {
@@ -194,18 +195,18 @@ __global__ void __launch_bounds__(512, 1) k_c2r_nonlin(cplx* __restrict__ psi, c
                 po[2 * m + 1] = phi.y;
                 continue;
             }
-            cplx a[2] = {p[2 * m], p[2 * m + 1]};
+            DT a[2] = {p[2 * m], p[2 * m + 1]};
             const double ph[2] = {phi.x, phi.y};
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
                 const double dens = s2 * cabs2(a[t]);
                 const double V = 0.5 * (vxy + __ldg(&A.vz[2 * m + t]));
-                if (MODE == 2) {
+                if constexpr (MODE == 2) {
                     acc[0] += V * dens;
                     acc[1] += dens * dens;
                     acc[2] += ph[t] * dens;
                     acc[3] += dens;
-                } else {
+                } else if constexpr (sizeof(DT) == sizeof(cplx)) {
                     const double H = V + A.g * dens + A.gdd * ph[t];
                     if (MODE == 0) {
                         const double f = exp(-A.dt * H) * s1;

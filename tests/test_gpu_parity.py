@@ -266,25 +266,96 @@ def test_step_host_matches_device_path(gpu):
 
 
 @pytest.mark.parametrize("mode", [0, 1])
-@pytest.mark.parametrize("env", ["DGPE_GENERIC=1", "DGPE_TMA=0", "DGPE_TMA=2", "DGPE_GRAPH=0", "DGPE_PREFETCH=0"])
-def test_kernel_variants_agree(gpu, monkeypatch, mode, env):
-    """The library carries two kernel sets (specialised and generic) and switches for
-    A/B runs; every variant must give the same step to rounding (different summation orders only)."""
+@pytest.mark.parametrize("opt", [{"generic": 1}, {"tma": 0}, {"tma": 2}, {"graph": 0}, {"prefetch": 0}, {"tma_fft": 0}])
+def test_kernel_variants_agree(gpu, mode, opt):
+    """The library carries two kernel sets (specialised and generic) and dgpe_create_ex options
+    for A/B runs; every variant must give the same step to rounding (different summation orders only)."""
     shape = (64, 384, 128)
     args = (*shape, 0.3, 0.25, 0.2, 0.004, 1.0, 0.7, 1.3, 5.0, 3.0, mode)
     psi = inputs.random_state(shape, 21) * 0.05
     ref = dev(psi)
     gpu.Dgpe(*args).step(ref, 3)
-    name, val = env.split("=")
-    monkeypatch.setenv(name, val)
     alt = dev(psi)
-    gpu.Dgpe(*args).step(alt, 3)
+    gpu.Dgpe(*args, options=opt).step(alt, 3)
     assert float((alt - ref).abs().max()) <= 1e-13
 
 
 @pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("shape,group", [((64, 64, 64), -1), ((64, 64, 64), 1), ((128, 128, 24), 2), ((192, 192, 20), 1),
+                                         ((256, 256, 36), -1), ((320, 320, 18), 1), ((384, 384, 20), 1), ((480, 480, 12), 1),
+                                         ((512, 512, 20), 1), ((512, 512, 48), 2)])
+def test_fused_fft_slab_kernel_agrees(gpu, oracle, mode, shape, group):
+    """K2 + K3 + K4 as the one L2-resident slab kernel (xyfft_fused.cuh; the default when nx == ny is one of its
+    lengths) against the three separate launches, and against the oracle's Phi: every fused length, ragged last
+    slabs (nz/2+1 = 33, 13, 11, 19, 10, 7, 25 bins: 1 to 7 valid columns in the last slab), one and several slabs
+    per group."""
+    args = (*shape, 0.3, 0.25, 0.2, 0.004, 1.0, 0.7, 1.3, 5.0, 3.0, mode)
+    psi = inputs.random_state(shape, 29) * 0.2
+    ref = oracle.Oracle(*args).dipolar(np.ascontiguousarray(psi.real ** 2 + psi.imag ** 2))
+    out = []
+    for opt in ({"fused_fft": 0}, {"fused_fft": 1, "fused_group": group}):
+        G = gpu.Dgpe(*args, options=opt)
+        assert ("K2+K3+K4" in " ".join(n for n, _, _ in G.step_profile(dev(psi), 1))) == bool(opt["fused_fft"])
+        phi = G.dipolar(dev(psi)).cpu().numpy()
+        assert np.max(np.abs(phi - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref))), opt
+        t = dev(psi)
+        G.step(t, 4)                # eager first step, then graph replays (the queue counters are reset per launch)
+        out.append((phi, t.cpu().numpy()))
+    assert np.max(np.abs(out[0][0] - out[1][0])) <= 1e-13 * max(1.0, np.max(np.abs(ref)))
+    assert np.max(np.abs(out[0][1] - out[1][1])) <= 1e-13
+
+
+def test_fused_fft_is_the_default_where_it_applies(gpu):
+    cfg = inputs.CONFIGS["C1"]
+    names = [n for n, _, _ in gpu.Dgpe(*cfg.create_args()).step_profile(dev(inputs.initial_state(cfg)), 1)]
+    assert len(names) == 5 and "K2+K3+K4" in names[1]
+    G = gpu.Dgpe(64, 48, 64, 0.25, 0.25, 0.25, 0.005, 1.0, 1.0, 1.0, 20.0, 5.0, 0)      # nx != ny: three launches
+    assert G.launches_per_step == 7
+
+
+def test_handles_of_different_sizes_alive_together(gpu, oracle):
+    """The shared-memory opt-in of a kernel is per process and device, not per handle: creating a small
+    handle must not lower the limit a larger live handle launches with -- generic kernels (972 = 2^2 3^5 has no
+    specialised kernel), the observables' K5, and the specialised ones."""
+    big_shape, small_shape = (8, 8, 972), (8, 8, 8)
+    phys = (0.3, 0.25, 0.2, 0.004, 1.0, 0.7, 1.3, 5.0, 3.0, 0)
+    big = gpu.Dgpe(*big_shape, *phys)
+    psi = inputs.random_state(big_shape, 31) * 0.3
+    t = dev(psi)
+    big.step(t, 1)
+    small = gpu.Dgpe(*small_shape, *phys)
+    ts = dev(inputs.random_state(small_shape, 32) * 0.3)
+    small.step(ts, 1)
+    small.chempot(ts)
+    # the large handle still launches: step, observables, dipolar
+    big.step(t, 1)
+    a = psi.copy()
+    O = oracle.Oracle(*big_shape, *phys)
+    O.step(a, 2)
+    assert np.max(np.abs(t.cpu().numpy() - a)) <= TOL_1
+    assert abs(big.chempot(t) - O.chempot(a)) <= TOL_OBS * abs(O.chempot(a))
+    ref = O.dipolar(np.ascontiguousarray(a.real ** 2 + a.imag ** 2))
+    assert np.max(np.abs(big.dipolar(t).cpu().numpy() - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref)))
+    # and the same with the specialised 512-point kernels next to a 64-point handle
+    big2 = gpu.Dgpe(512, 8, 8, *phys)
+    t2 = dev(inputs.random_state((512, 8, 8), 33) * 0.3)
+    big2.step(t2, 1)
+    gpu.Dgpe(64, 8, 8, *phys).step(dev(inputs.random_state((64, 8, 8), 34) * 0.3), 1)
+    assert big2.step(t2, 1) == gpu.OK
+
+
+def test_create_reports_the_error_code(gpu):
+    with pytest.raises(gpu.DgpeError) as e:
+        gpu.Dgpe(8, 8, 10, 0.1, 0.1, 0.1, 0.01, 1.0, 1.0, 1.0, 1.0, 1.0, gpu.IMAG_RPSI)      # nz = 10: no z-line kernel
+    assert e.value.code == gpu.ERR_UNSUPPORTED
+    with pytest.raises(gpu.DgpeError) as e:
+        gpu.Dgpe(8, 8, 17, 0.1, 0.1, 0.1, 0.01, 1.0, 1.0, 1.0, 1.0, 1.0, 0)
+    assert e.value.code == gpu.ERR_ARG
+
+
+@pytest.mark.parametrize("mode", [0, 1])
 @pytest.mark.parametrize("nx", [384, 480, 512, 640])
-def test_k3_tma_pipeline_agrees(gpu, oracle, monkeypatch, nx, mode):
+def test_k3_tma_pipeline_agrees(gpu, oracle, nx, mode):
     """K3 (FFT_x, Udd~, IFFT_x) has a thread-loading and a TMA-pipelined kernel (the default from nx = 640 up,
     DESIGN.md section 6): each forced in turn gives the same Phi, and that Phi is the oracle's."""
     shape = (nx, 12, 64)            # 12 * 33 = 396 flattened (ky, kz) columns: a ragged last tile (396 = 49 * 8 + 4)
@@ -292,9 +363,8 @@ def test_k3_tma_pipeline_agrees(gpu, oracle, monkeypatch, nx, mode):
     psi = inputs.random_state(shape, 23) * 0.3
     ref = oracle.Oracle(*args).dipolar(np.ascontiguousarray(psi.real ** 2 + psi.imag ** 2))
     out = []
-    for val in ("0", "1"):
-        monkeypatch.setenv("DGPE_TMA_K3", val)
-        G = gpu.Dgpe(*args)
+    for val in (0, 1):
+        G = gpu.Dgpe(*args, options={"tma_k3": val})
         out.append(G.dipolar(dev(psi)).cpu().numpy())
         assert np.max(np.abs(out[-1] - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref))), val
         t = dev(psi)
