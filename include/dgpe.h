@@ -96,11 +96,7 @@ typedef struct dgpe_options {
     int prefetch;     /* mask of kernel families with the L2 prefetch of the next residency:
                          1 z lines, 2 y sweep, 4 x sweep, 8 y FFT, 16 x FFT                                 */
     int pf_mult;      /* prefetch distance in units of one residency (default 1)                            */
-    int fused_fft;    /* 0: K2, K3, K4 as three launches; 1: as one persistent kernel over L2-resident kz
-                         slabs whenever the shape allows (default: when two slab groups fit L2)             */
-    int fused_group;  /* kz slabs per group of the fused kernel's queue (default: from the slab size)       */
-    int fused_sweep;  /* 0: x and y sweeps as two launches; 1: one persistent kernel over L2-resident z slabs */
-    int reserved[6];  /* set to -1 */
+    int reserved[9];  /* set to -1 */
 } dgpe_options;
 dgpe_handle* dgpe_create_ex(int nx, int ny, int nz, double dx, double dy, double dz, double dt,
                             double gamma, double nu, double lambda, double g, double gdd, int mode,

@@ -27,7 +27,6 @@
 #include "xysweep.cuh"
 #include "xysweep_tma.cuh"
 #include "xyfft_tma.cuh"
-#include "xyfft_fused.cuh"
 #include "zline.cuh"
 
 using namespace dgpe;
@@ -97,14 +96,8 @@ struct dgpe_handle {
     bool use_tma_x = false;          // DGPE_TMA=2: TMA on the x axis at every length (A/B)
     bool use_tma = true;             // DGPE_TMA=0: the x/y sweeps load and store through the threads (k_sweep_xy)
     bool zfast = false;              // warp-per-line z kernels (zline.cuh) and the fused step order z, x, y
-    // K2 + K3 + K4 as one persistent kernel over L2-resident kz slabs (xyfft_fused.cuh): nx == ny, one of the
-    // specialised lengths, two slab groups fit L2.  DGPE_FUSED_FFT=0 keeps the three launches (A/B runs).
     dgpe_options opt;                // as given to dgpe_create_ex (all -1 from dgpe_create)
     int device = 0;                  // the CUDA device the handle lives on (current at creation)
-    bool fused_fft = false;
-    int fused_nslab = 0, fused_nunits = 0, fused_gs = 0;
-    int* fused_units = nullptr;          // device: queue order of the (phase, slab) units
-    unsigned int* fused_ctr = nullptr;   // device: queue head + 2 nslab tile counters
 
     cplx* spec = nullptr;                       // [nx][ny][nzh]
     FftPlan plan_x{}, plan_y{}, plan_zh{};      // transform lengths nx, ny, nz/2
@@ -132,7 +125,6 @@ struct dgpe_handle {
 };
 
 static bool z_specialised(int nz);
-static bool fused_fft_supported(int nx, int ny);
 
 static int threads_for(int nbf)
 {
@@ -316,7 +308,8 @@ static int kernel_setup(const void* func, int threads, size_t smem, int* ctas_pe
     CU(cudaGetDevice(&dev));
     std::lock_guard<std::mutex> lock(mu);
     size_t& optin = allowed[std::make_pair(func, dev)];
-    if (smem > 48 * 1024 && smem > optin) {
+    // (the limit counts static shared memory too: opt in from 40 KB of dynamic memory up)
+    if (smem > 40 * 1024 && smem > optin) {
         CU(cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         optin = smem;
     }
@@ -422,34 +415,6 @@ static int init_handle(dgpe_handle* h)
     h->owned.push_back(h->d_out);
     CU(cudaMallocHost(&h->h_out, sizeof(double) * 16));
 
-    // K2 + K3 + K4 through L2 (xyfft_fused.cuh): queue order of the (phase, slab) units,
-    //   A(g), C(g-1), B(g), A(g+1), C(g), B(g+1), ...   over groups g of `gs` neighbouring kz slabs,
-    // so that two groups are alive in L2 at a time and a phase's producer was handed out a whole phase earlier.
-    if (fused_fft_supported(nx, ny) && !h->force_generic && h->opt.fused_fft != 0) {
-        const int nslab = (nzh + TILE_COLS - 1) / TILE_COLS;
-        const double slab_bytes = (double)nx * ny * TILE_COLS * sizeof(cplx);
-        // group size: two groups within ~70 MB of the 126 MB L2 (one 33.5 MB slab per group at 512^2), and
-        // enough tiles per phase to fill the machine on the small grids
-        int gs = (int)(35.0e6 / slab_bytes);
-        gs = std::max(1, std::min(gs, nslab));
-        if (h->opt.fused_group > 0) gs = std::min(h->opt.fused_group, nslab);
-        if (2.0 * gs * slab_bytes <= 100.0e6 || h->opt.fused_fft == 1) {
-            std::vector<int> units;
-            const int G = (nslab + gs - 1) / gs;
-            auto emit = [&](int phase, int g) {
-                if (g < 0 || g >= G) return;
-                for (int sl = g * gs; sl < std::min(nslab, (g + 1) * gs); ++sl) units.push_back(phase | (sl << 2));
-            };
-            for (int k = 0; k <= G; ++k) { emit(0, k); emit(2, k - 1); emit(1, k); }
-            h->fused_nslab = nslab;
-            h->fused_nunits = (int)units.size();
-            h->fused_gs = gs;
-            if ((rc = upload(h, units, &h->fused_units))) return rc;
-            CU(cudaMalloc(&h->fused_ctr, sizeof(unsigned int) * (size_t)(1 + 2 * nslab)));
-            h->owned.push_back(h->fused_ctr);
-            h->fused_fft = true;
-        }
-    }
     return DGPE_OK;
 }
 
@@ -938,56 +903,11 @@ static int launch_fft_x_udd(dgpe_handle* h)
     return check_launch("k_fft_x_udd");
 }
 
-// ---- K2 + K3 + K4 as one launch over L2-resident kz slabs (xyfft_fused.cuh) ----
-#define DGPE_FUSED_SIZES(X) X(64) X(128) X(192) X(256) X(320) X(384) X(480) X(512)
-
-static bool fused_fft_supported(int nx, int ny)
-{
-    if (nx != ny) return false;
-    switch (nx) {
-#define X(NN) case NN:
-        DGPE_FUSED_SIZES(X)
-#undef X
-        return true;
-        default: return false;
-    }
-}
-
-template <int N>
-static int launch_fft_fused_n(dgpe_handle* h)
-{
-    auto kern = k_fft_yxy<N>;
-    const size_t smem = (size_t)N * TILE_COLS * sizeof(cplx);
-    int ctas_per_sm = 0;
-    int rc = kernel_setup((const void*)kern, xy_threads<N>(), smem, &ctas_per_sm);
-    if (rc) return rc;
-    CU(cudaMemsetAsync(h->fused_ctr, 0, sizeof(unsigned int) * (size_t)(1 + 2 * h->fused_nslab), h->stream));
-    const int nitems = h->fused_nunits * N;      // one CTA per tile; the CTAs claim their tiles in queue order
-    FusedWalk W;
-    W.ny = h->ny; W.nzh = h->nzh; W.nslab = h->fused_nslab; W.nunits = h->fused_nunits;
-    W.units = h->fused_units; W.head = h->fused_ctr; W.done = h->fused_ctr + 1;
-    W.pf_items = (h->prefetch & PF_FFT_Y) ? h->pf_mult * ctas_per_sm * h->num_sms : 0;
-    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 2.0 * 3.14159265358979323846264338327950288 / ((double)h->nx * h->dx), 1.0 / (double)h->N, 0};
-    kern<<<nitems, xy_threads<N>(), smem, h->stream>>>(h->spec, W, h->tw_y, U);
-    return check_launch("k_fft_yxy");
-}
-
-static int launch_fft_fused(dgpe_handle* h)
-{
-    switch (h->nx) {
-#define X(NN) case NN: return launch_fft_fused_n<NN>(h);
-        DGPE_FUSED_SIZES(X)
-#undef X
-        default: return fail(DGPE_ERR_UNSUPPORTED, "no fused FFT kernel for nx = ny = %d", h->nx);
-    }
-}
-
 // K1..K4: spec <- Udd~(k)/N * FFT(s2 |psi|^2), transformed back along x and y
 static int launch_dipolar_spectrum(dgpe_handle* h, const cplx* psi)
 {
     int rc;
     if ((rc = launch_k1(h, psi))) return rc;
-    if (h->fused_fft) return launch_fft_fused(h);
     if ((rc = launch_fft_y(h, false))) return rc;
     if ((rc = launch_fft_x_udd(h))) return rc;
     return launch_fft_y(h, true);
@@ -1175,8 +1095,7 @@ static int set_scal(dgpe_handle* h, int clear_bad)
 
 // One step = 8 kernels in the order of the method (K1..K5, sweeps x, y, z); 7 when the z-line kernels are
 // available: the z sweep then runs fused into K5 and the sweeps go z, x, y (the three 1-D Cayley operators
-// commute: R#26); 5 when K2, K3, K4 also run as the one L2-resident slab kernel.  The norm is folded into the
-// last sweep either way.  `mark` is called after each launch with the kernel index.
+// commute: R#26).  The norm is folded into the last sweep either way.  `mark` is called after each launch with the kernel index.
 struct StepKernel { const char* name; double bytes; };
 
 // the kernels of one step AS BUILT with their algorithmic bytes (each array read once and written once per pass)
@@ -1186,13 +1105,9 @@ static std::vector<StepKernel> step_kernels(const dgpe_handle* h)
     const double N = (h->rpsi ? 0.5 : 1.0) * (double)h->N;      // in units of 16 bytes of psi
     std::vector<StepKernel> k;
     k.push_back({"K1 dens_r2c(z)", 16.0 * N + S});
-    if (h->fused_fft) {
-        k.push_back({"K2+K3+K4 fft_y.fft_x*Udd*ifft_x.ifft_y (L2-resident slabs)", 2.0 * S});
-    } else {
-        k.push_back({"K2 fft_y fwd", 2.0 * S});
-        k.push_back({"K3 fft_x*Udd*ifft_x", 2.0 * S});
-        k.push_back({"K4 fft_y inv", 2.0 * S});
-    }
+    k.push_back({"K2 fft_y fwd", 2.0 * S});
+    k.push_back({"K3 fft_x*Udd*ifft_x", 2.0 * S});
+    k.push_back({"K4 fft_y inv", 2.0 * S});
     if (h->zfast) {
         k.push_back({"K5+K8 c2r(z)+nonlinear+sweep_z", S + 32.0 * N});     // the fused z sweep adds no traffic
         k.push_back({"K6 sweep_x", 32.0 * N});
@@ -1213,17 +1128,12 @@ static int one_step(dgpe_handle* h, cplx* psi, Mark mark)
     int rc, k = 0;
     if ((rc = launch_k1(h, psi))) return rc;
     mark(k++);
-    if (h->fused_fft) {
-        if ((rc = launch_fft_fused(h))) return rc;
-        mark(k++);
-    } else {
-        if ((rc = launch_fft_y(h, false))) return rc;
-        mark(k++);
-        if ((rc = launch_fft_x_udd(h))) return rc;
-        mark(k++);
-        if ((rc = launch_fft_y(h, true))) return rc;
-        mark(k++);
-    }
+    if ((rc = launch_fft_y(h, false))) return rc;
+    mark(k++);
+    if ((rc = launch_fft_x_udd(h))) return rc;
+    mark(k++);
+    if ((rc = launch_fft_y(h, true))) return rc;
+    mark(k++);
     if (h->zfast) {
         if ((rc = launch_z_main(h, psi, 1, nullptr))) return rc;
         mark(k++);

@@ -280,39 +280,6 @@ def test_kernel_variants_agree(gpu, mode, opt):
     assert float((alt - ref).abs().max()) <= 1e-13
 
 
-@pytest.mark.parametrize("mode", [0, 1])
-@pytest.mark.parametrize("shape,group", [((64, 64, 64), -1), ((64, 64, 64), 1), ((128, 128, 24), 2), ((192, 192, 20), 1),
-                                         ((256, 256, 36), -1), ((320, 320, 18), 1), ((384, 384, 20), 1), ((480, 480, 12), 1),
-                                         ((512, 512, 20), 1), ((512, 512, 48), 2)])
-def test_fused_fft_slab_kernel_agrees(gpu, oracle, mode, shape, group):
-    """K2 + K3 + K4 as the one L2-resident slab kernel (xyfft_fused.cuh; the default when nx == ny is one of its
-    lengths) against the three separate launches, and against the oracle's Phi: every fused length, ragged last
-    slabs (nz/2+1 = 33, 13, 11, 19, 10, 7, 25 bins: 1 to 7 valid columns in the last slab), one and several slabs
-    per group."""
-    args = (*shape, 0.3, 0.25, 0.2, 0.004, 1.0, 0.7, 1.3, 5.0, 3.0, mode)
-    psi = inputs.random_state(shape, 29) * 0.2
-    ref = oracle.Oracle(*args).dipolar(np.ascontiguousarray(psi.real ** 2 + psi.imag ** 2))
-    out = []
-    for opt in ({"fused_fft": 0}, {"fused_fft": 1, "fused_group": group}):
-        G = gpu.Dgpe(*args, options=opt)
-        assert ("K2+K3+K4" in " ".join(n for n, _, _ in G.step_profile(dev(psi), 1))) == bool(opt["fused_fft"])
-        phi = G.dipolar(dev(psi)).cpu().numpy()
-        assert np.max(np.abs(phi - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref))), opt
-        t = dev(psi)
-        G.step(t, 4)                # eager first step, then graph replays (the queue counters are reset per launch)
-        out.append((phi, t.cpu().numpy()))
-    assert np.max(np.abs(out[0][0] - out[1][0])) <= 1e-13 * max(1.0, np.max(np.abs(ref)))
-    assert np.max(np.abs(out[0][1] - out[1][1])) <= 1e-13
-
-
-def test_fused_fft_is_the_default_where_it_applies(gpu):
-    cfg = inputs.CONFIGS["C1"]
-    names = [n for n, _, _ in gpu.Dgpe(*cfg.create_args()).step_profile(dev(inputs.initial_state(cfg)), 1)]
-    assert len(names) == 5 and "K2+K3+K4" in names[1]
-    G = gpu.Dgpe(64, 48, 64, 0.25, 0.25, 0.25, 0.005, 1.0, 1.0, 1.0, 20.0, 5.0, 0)      # nx != ny: three launches
-    assert G.launches_per_step == 7
-
-
 def test_handles_of_different_sizes_alive_together(gpu, oracle):
     """The shared-memory opt-in of a kernel is per process and device, not per handle: creating a small
     handle must not lower the limit a larger live handle launches with -- generic kernels (972 = 2^2 3^5 has no
