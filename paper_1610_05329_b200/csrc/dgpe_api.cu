@@ -69,6 +69,7 @@ struct AxisSweep {
     void* Bch = nullptr;
     std::vector<std::complex<double>> h_inv, h_cc, h_F, h_Gm;   // host copies (kernel-parameter tables of the z sweep)
     bool consttab = false;   // chunk 0 + one converged chunk describe the whole line (zline.cuh ZTabs)
+    void* ztab = nullptr;    // device, 8 Lc entries: [inv, cc, F, Gm] of chunk 0, then of the converged chunk (consttab only)
 };
 
 enum { PF_Z = 1, PF_SWEEP_Y = 2, PF_SWEEP_X = 4, PF_FFT_Y = 8, PF_FFT_X = 16 };
@@ -287,6 +288,16 @@ static int build_sweep(dgpe_handle* h, AxisSweep* S, int n, std::complex<double>
     if ((rc = conv(Gm, &S->Gm))) return rc;
     if ((rc = conv(A, &S->Ach))) return rc;
     if ((rc = conv(B, &S->Bch))) return rc;
+    if (S->consttab) {
+        const int lc2 = S->Lc, u0 = (S->G >= 2) ? 1 + lc2 : 1;
+        std::vector<C> zt(8 * (size_t)lc2, C(0));
+        for (int i = 0; i < lc2; ++i) {
+            const int a = std::min(1 + i, n - 1), b = std::min(u0 + i, n - 1);      // entries past n-2 are zero and unused
+            zt[i] = inv[a]; zt[lc2 + i] = cc[a]; zt[2 * lc2 + i] = F[b]; zt[3 * lc2 + i] = Gm[a];
+            zt[4 * lc2 + i] = inv[b]; zt[5 * lc2 + i] = cc[b]; zt[6 * lc2 + i] = F[b]; zt[7 * lc2 + i] = Gm[b];
+        }
+        if ((rc = conv(zt, &S->ztab))) return rc;
+    }
     return DGPE_OK;
 }
 
@@ -602,7 +613,7 @@ static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
     T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb; T.gU = S.gU;
     if (SWEEP && (S.Lc != LC || S.G > ZGeom<NZ>::T)) return fail(DGPE_ERR_CUDA, "z sweep tables do not match the z-line kernel");
     ChunkTabs<CT, LC> P;
-    fill_chunk_tabs<CT, LC>(S, SWEEP && CONSTTAB, &P);
+    fill_chunk_tabs<CT, LC>(S, SWEEP && CONSTTAB && sizeof(DT) == sizeof(double), &P);      // real-valued psi only (zline.cuh)
     ZMainArgs Z;
     Z.nlines = h->nx * h->ny; Z.ny = h->ny;
     Z.dt = h->dt; Z.g = h->g; Z.gdd = h->gdd;
@@ -610,7 +621,8 @@ static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
     Z.dz = h->dz; Z.lam2 = h->lambda * h->lambda;
     Z.scal = h->scal; Z.tw = h->tw_zh; Z.tws = h->tw_split; Z.phi_out = phi_out;
     Z.pf_lines = (h->prefetch & PF_Z) ? h->pf_mult * ctas_per_sm * h->num_sms * LINES : 0;
-    kern<<<(Z.nlines + LINES - 1) / LINES, 32 * WARPS, smem, h->stream>>>((DT*)psi, h->spec, Z, T, P);
+    if (SWEEP && CONSTTAB && !S.ztab) return fail(DGPE_ERR_CUDA, "z sweep tables were not built for the z-line kernel");
+    kern<<<(Z.nlines + LINES - 1) / LINES, 32 * WARPS, smem, h->stream>>>((DT*)psi, h->spec, Z, T, (const CT*)S.ztab, P);
     return check_launch("k_z_main");
 }
 

@@ -73,8 +73,7 @@ k_sweep_xy(cplx* __restrict__ psi, LineMap map, SweepTables<CT> T, SweepFold fol
         if (work && i < cnt) {
             // e_j = inv_j (d_j + r e_{j-1}) written as inv_j d_j + (r inv_j) e_{j-1}, r inv_j = -c_j: one
             // dependent fma per unknown instead of an fma and a multiply
-            cplx d = coef_mul(T.r, cadd(p[i], p[i + 2]));
-            d = coef_fma(T.omr2, p[i + 1], d);
+            const cplx d = cn_rhs(T.r, T.omr2, p[i], p[i + 1], p[i + 2]);
             e = coef_fma(coef_neg(t_cc(i)), e, coef_mul(t_inv(i), d));
             ev[i] = e;
         }

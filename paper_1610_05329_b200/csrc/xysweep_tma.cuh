@@ -118,8 +118,7 @@ k_sweep_tma(const __grid_constant__ CUtensorMap tmap, TmaWalk W, SweepTables<CT>
             for (int i = 0; i < LC; ++i) {
                 ev[i] = mk(0.0, 0.0);
                 if (work && i < cnt) {
-                    cplx d = coef_mul(T.r, cadd(p[i], p[i + 2]));
-                    d = coef_fma(T.omr2, p[i + 1], d);
+                    const cplx d = cn_rhs(T.r, T.omr2, p[i], p[i + 1], p[i + 2]);
                     e = coef_fma(coef_neg(t_cc(M, i)), e, coef_mul(t_inv(M, i), d));
                     ev[i] = e;
                 }

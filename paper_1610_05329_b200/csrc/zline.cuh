@@ -27,6 +27,7 @@
 #include "ctfft.cuh"
 #include "sweep.cuh"
 #include "tma.cuh"
+#include <type_traits>
 
 namespace dgpe {
 
@@ -239,7 +240,7 @@ __device__ __forceinline__ void bulk_store(void* gdst, const void* smem_src, uns
 template <int NZ, typename CT, typename DT, int SPEC, bool SWEEP, bool CONSTTAB, int WARPS, int MINB>
 __global__ void __launch_bounds__(32 * WARPS, MINB)
 k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, SweepTables<CT> T,
-         const __grid_constant__ ChunkTabs<CT, ZGeom<NZ>::LC> P)
+         const CT* __restrict__ ptab, const __grid_constant__ ChunkTabs<CT, ZGeom<NZ>::LC> P)
 {
     using G = ZGeom<NZ>;
     constexpr int M = G::M, L = ct::npass(M), LC = G::LC, TL = G::T, LPW = G::LPW;
@@ -354,7 +355,11 @@ k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Sweep
         s2 = Z.scal[SC_S2];
         s1 = Z.scal[SC_S1];
     }
-    auto upd = [&](int e) -> DT {
+    // PRECISE = false: the branch-free sincos_fast; it is exact to 2e-16 below SINCOS_FAST_LIMIT, and `big` records
+    // an argument at or beyond it (or a NaN), for which the caller evaluates the point again with PRECISE = true
+    // (the library's sincos with its exact reduction) -- never taken for the phases of a physical state
+    bool big = false;
+    auto upd_as = [&](int e, auto precise) -> DT {
         DT a = A[e];
         if constexpr (SPEC == ZS_IMAG || SPEC == ZS_REAL) {
             const double z = (double)(e - NZ / 2) * Z.dz;          // R#6
@@ -365,13 +370,20 @@ k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Sweep
                 const double f = exp(-Z.dt * H) * s1;
                 a = coef_mul(f, a);
             } else {
+                const double th = Z.dt * H;
                 double sn, cs;
-                sincos(Z.dt * H, &sn, &cs);
+                if constexpr (decltype(precise)::value) {
+                    sincos(th, &sn, &cs);
+                } else {
+                    sincos_fast(th, &sn, &cs);
+                    big |= !(fabs(th) < SINCOS_FAST_LIMIT);
+                }
                 a = mk(cs * a.x + sn * a.y, cs * a.y - sn * a.x);
             }
         }
         return a;
     };
+    auto upd = [&](int e) -> DT { return upd_as(e, std::false_type()); };
 
     const int s = 1 + lane * LC;
     const int cnt = min(LC, NZ - 1 - s);                  // unknowns of this lane's chunk (<= 0: idle lane)
@@ -380,11 +392,37 @@ k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Sweep
         // table base of this lane (CONSTTAB = false): away from the left wall the elimination factors have
         // converged, so the interior chunks share one set of entries (T.gU) -- one broadcast address
         const int sT = (lane >= T.gU && lane < Gn - 1) ? 1 + T.gU * LC : s;
+        // CONSTTAB: the Thomas factors of chunk 0 and of the converged chunk as ONE compact table of 8 LC entries
+        // (ptab, built on the host: [inv, cc, F, Gm] of chunk 0, then of the converged chunk; F of chunk 0 multiplies a
+        // zero inflow), read through L1 with the lane-0 / other-lanes choice in the address: one load per factor, two
+        // addresses per warp.  (As kernel parameters every factor cost three LDC per double -- one for chunk 0, two
+        // predicated ones for the converged chunk -- and the constant-load unit was the busiest pipe of the real-time
+        // kernel: 60 % in ncu.  A copy in shared memory costs the 16th resident line at nz = 256 and 512.)
+        // Real-valued psi (every quantity one double, half the factors): there the kernel parameters stay faster
+        // (measured at 512^3: 0.709 vs 0.738 ms).
+        constexpr bool PARAMTAB = CONSTTAB && sizeof(DT) == sizeof(double);
+        const CT* tb = ptab + (lane == 0 ? 0 : 4 * LC);
         const bool l0 = lane == 0;
-        auto t_inv = [&](int i) { if constexpr (CONSTTAB) return l0 ? P.inv0[i] : P.invU[i]; else return __ldg(&T.inv[sT + i]); };
-        auto t_cc = [&](int i) { if constexpr (CONSTTAB) return l0 ? P.cc0[i] : P.ccU[i]; else return __ldg(&T.cc[sT + i]); };
-        auto t_F = [&](int i) { if constexpr (CONSTTAB) return P.fU[i]; else return __ldg(&T.F[sT + i]); };
-        auto t_Gm = [&](int i) { if constexpr (CONSTTAB) return l0 ? P.gm0[i] : P.gmU[i]; else return __ldg(&T.Gm[sT + i]); };
+        auto t_inv = [&](int i) {
+            if constexpr (PARAMTAB) return l0 ? P.inv0[i] : P.invU[i];
+            else if constexpr (CONSTTAB) return __ldg(&tb[i]);
+            else return __ldg(&T.inv[sT + i]);
+        };
+        auto t_cc = [&](int i) {
+            if constexpr (PARAMTAB) return l0 ? P.cc0[i] : P.ccU[i];
+            else if constexpr (CONSTTAB) return __ldg(&tb[LC + i]);
+            else return __ldg(&T.cc[sT + i]);
+        };
+        auto t_F = [&](int i) {
+            if constexpr (PARAMTAB) return P.fU[i];
+            else if constexpr (CONSTTAB) return __ldg(&tb[2 * LC + i]);
+            else return __ldg(&T.F[sT + i]);
+        };
+        auto t_Gm = [&](int i) {
+            if constexpr (PARAMTAB) return l0 ? P.gm0[i] : P.gmU[i];
+            else if constexpr (CONSTTAB) return __ldg(&tb[3 * LC + i]);
+            else return __ldg(&T.Gm[sT + i]);
+        };
 
         // ---- A: nonlinear update on the fly + local forward elimination with zero inflow; the end nodes
         //      of the line are read as zero (R#7, R#8).
@@ -399,6 +437,19 @@ k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Sweep
             const DT v = upd(min(j, NZ - 1));
             pv[i] = el_sel(j <= NZ - 2, v, zero);
         }
+        if constexpr (SPEC == ZS_REAL) {
+            if (big) {                                   // rare: a phase beyond the fast reduction's range
+#pragma unroll 1
+                for (int i = 1; i <= LC; ++i) {
+                    const int j = s - 1 + i;
+                    const DT v = upd_as(min(j, NZ - 1), std::true_type());
+                    const DT w = el_sel(j <= NZ - 2, v, zero);
+                    // pv is a register array: select the entry without dynamic indexing
+#pragma unroll
+                    for (int u = 1; u <= LC; ++u) pv[u] = el_sel(u == i, w, pv[u]);
+                }
+            }
+        }
         {
             const DT up = shfl_ct<TL>(pv[LC], (lane + TL - 1) & (TL - 1)), dn = shfl_ct<TL>(pv[1], (lane + 1) & (TL - 1));
             pv[0] = (lane == 0) ? zero : up;
@@ -409,8 +460,7 @@ k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Sweep
 #pragma unroll
         for (int i = 0; i < LC; ++i) {
             // inv_j (d_j + r e_{j-1}) = inv_j d_j + (-c_j) e_{j-1}: one dependent fma per unknown
-            DT d = coef_mul(T.r, cadd(pv[i], pv[i + 2]));
-            d = coef_fma(T.omr2, pv[i + 1], d);
+            const DT d = cn_rhs(T.r, T.omr2, pv[i], pv[i + 1], pv[i + 2]);
             const DT en = coef_fma(coef_neg(t_cc(i)), e, coef_mul(t_inv(i), d));
             e = el_sel(i < cnt, en, e);
             ev[i] = e;
@@ -452,11 +502,18 @@ k_z_main(DT* __restrict__ psi, const cplx* __restrict__ spec, ZMainArgs Z, Sweep
         if (lane == TL - 1) A[NZ - 1] = zero;
     } else {
         // nonlinear update only (dgpe_nonlinear): every point of the line, end nodes included
+        // (dgpe_nonlinear, not the step: same fast sincos, the fallback decided point by point)
+        auto upd_checked = [&](int e) -> DT {
+            big = false;
+            DT v = upd(e);
+            if (big) v = upd_as(e, std::true_type());
+            return v;
+        };
 #pragma unroll
         for (int i = 0; i < LC; ++i)
-            if (i < cnt) A[s + i] = upd(s + i);
-        if (lane == 0) A[0] = upd(0);
-        if (lane == TL - 1) A[NZ - 1] = upd(NZ - 1);
+            if (i < cnt) A[s + i] = upd_checked(s + i);
+        if (lane == 0) A[0] = upd_checked(0);
+        if (lane == TL - 1) A[NZ - 1] = upd_checked(NZ - 1);
     }
 
     // ---- the line goes back by one bulk store ----

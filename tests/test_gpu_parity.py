@@ -280,6 +280,47 @@ def test_kernel_variants_agree(gpu, mode, opt):
     assert float((alt - ref).abs().max()) <= 1e-13
 
 
+@pytest.mark.parametrize("shape", [(8, 8, 64), (8, 6, 384), (8, 8, 100)])
+@pytest.mark.parametrize("theta_max", [20.0, 3.0e4, 5.0e9])
+def test_real_time_phase_range_of_the_fast_sincos(gpu, oracle, shape, theta_max):
+    """Real time: exp(-i dt H) through the branch-free sincos of the z-line kernels (common.cuh sincos_fast) against the
+    oracle's libm, for phases dt H up to 20 rad (every config stays below: <= 1e-12), up to 3e4 rad (fast reduction,
+    many quadrants) and beyond 2^30 rad, where the kernel switches to the library routine.  The two sides add the
+    terms of H in different orders, so theta itself differs by an ulp: the bound scales with theta.  (8, 8, 100) has
+    no z-line kernel: the generic K5 with the library's sincos."""
+    dt, g = 0.01, 50.0
+    psi = inputs.random_state(shape, 41)
+    nmax = float(np.max(np.abs(psi) ** 2))
+    psi *= np.sqrt(theta_max / (dt * g * nmax))                    # the largest phase is ~ theta_max
+    args = (*shape, 0.3, 0.25, 0.2, dt, 1.0, 0.7, 1.3, g, 0.0, 1)  # gdd = 0: the phase is dt (V + g |psi|^2)
+    G, O = gpu.Dgpe(*args), oracle.Oracle(*args)
+    amp = float(np.max(np.abs(psi)))
+    tol = max(1e-12, 16 * np.finfo(float).eps * theta_max * amp) if theta_max > 20.0 else 1e-12 * max(1.0, amp)
+    t, a = dev(psi), psi.copy()
+    G.nonlinear(t)
+    O.nonlinear(a)
+    assert np.max(np.abs(t.cpu().numpy() - a)) <= tol
+    t, a = dev(psi), psi.copy()
+    assert G.step(t, 1) == O.step(a, 1) == 0
+    assert np.max(np.abs(t.cpu().numpy() - a)) <= tol
+    assert abs(G.norm(t) / O.norm(a) - 1.0) <= 1e-12               # |exp(-i theta)| = 1 whatever theta
+
+
+def test_real_time_non_finite_phase_gives_nan_like_libm(gpu, oracle):
+    shape = (8, 8, 64)
+    args = (*shape, 0.3, 0.25, 0.2, 0.01, 1.0, 0.7, 1.3, 50.0, 0.0, 1)
+    psi = inputs.random_state(shape, 42)
+    psi[3, 4, 20] = 1e200                                          # |psi|^2 overflows: theta = inf, sin(inf) = NaN
+    G, O = gpu.Dgpe(*args), oracle.Oracle(*args)
+    t, a = dev(psi), psi.copy()
+    G.nonlinear(t)
+    O.nonlinear(a)
+    got = t.cpu().numpy()
+    assert np.array_equal(np.isnan(got.real) | np.isnan(got.imag), np.isnan(a.real) | np.isnan(a.imag))
+    ok = ~(np.isnan(a.real) | np.isnan(a.imag))
+    assert np.max(np.abs(got[ok] - a[ok])) <= 1e-12 and (~ok).sum() >= 1
+
+
 def test_handles_of_different_sizes_alive_together(gpu, oracle):
     """The shared-memory opt-in of a kernel is per process and device, not per handle: creating a small
     handle must not lower the limit a larger live handle launches with -- generic kernels (972 = 2^2 3^5 has no
