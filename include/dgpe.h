@@ -173,6 +173,45 @@ int dgpe_synchronize(dgpe_handle* h);
 double dgpe_bytes_per_step(const dgpe_handle* h);
 int dgpe_launches_per_step(const dgpe_handle* h);
 
+/*
+ * Slab-decomposed step -- one rank's share of a step distributed over `nranks` GPUs.
+ * The paper distributes the data "along NX": rank p owns the x slab psi[p NX/P .. (p+1) NX/P)[NY][NZ], whole
+ * lines along y and z, so the y and z passes and sweeps are local; "anything needing the whole NX extent" --
+ * the x pass of the dipolar convolution and the x sweep -- runs after an all-to-all exchange that leaves the data
+ * "locally transposed" as NX x (NY/P) x NZ, each rank sending every peer one (NX/P) x (NY/P) x NZ block,
+ * and is followed by the exchange back.  The library does the local stages and the strided packing of the blocks; the
+ * exchanges themselves belong to the caller (torch.distributed over NCCL in paper_1610_05329_b200/sharded.py, or local
+ * copies when all ranks are emulated on one device), which is why every buffer below is caller-owned:
+ *
+ *   begin
+ *   a(psi_x, spec_send)               K1, K2; spec_send[q] = block for rank q            -> all-to-all -> spec_y
+ *   b(spec_y)                         K3 in place on [NX][NY/P][NZ/2+1]                   -> all-to-all back -> spec_recv
+ *   c(spec_recv, psi_x, psi_send)     K4, K5 (+ z sweep), y sweep; psi_send[q] = block q  -> all-to-all -> psi_y
+ *   d(psi_y, norm_part)               x sweep in place on [NX][NY/P][NZ]; norm_part = own part of the norm
+ *                                                              -> all-to-all back -> psi_recv; all-reduce(norm_part) -> norm_total
+ *   e(psi_recv, psi_x, norm_total)    psi back in the x slab; scale factors of the next step
+ *   ... nsteps times ...; end(psi_x)  imaginary time: explicit rescale, DGPE_ERR_NONFINITE if a norm was 0/inf/NaN
+ *
+ * A buffer of blocks is [P][NX/P][NY/P][w] complex doubles (w = NZ/2+1 for the half-spectrum, NZ for psi); received from
+ * all ranks in rank order it IS the y slab [NX][NY/P][w], and the y slab is the send buffer of the way back.
+ * dgpe_slab_elems(s, spectrum) = (NX/P) NY w: the element count of every one of these buffers.
+ * Every pointer is a DEVICE pointer; all work is enqueued on the slab's stream; sweeps run in the order z, y, x (R#26).
+ * Errors as dgpe_create / dgpe_step; NX and NY must be divisible by nranks.  DGPE_IMAG and DGPE_REAL only.
+ */
+typedef struct dgpe_slab dgpe_slab;
+dgpe_slab* dgpe_slab_create(int nx, int ny, int nz, double dx, double dy, double dz, double dt, double gamma, double nu,
+                            double lambda, double g, double gdd, int mode, int nranks, int rank);
+void dgpe_slab_destroy(dgpe_slab* s);
+int dgpe_slab_set_stream(dgpe_slab* s, void* cuda_stream);
+long long dgpe_slab_elems(const dgpe_slab* s, int spectrum);
+int dgpe_slab_begin(dgpe_slab* s);
+int dgpe_slab_stage_a(dgpe_slab* s, const void* psi_x, void* spec_send);
+int dgpe_slab_stage_b(dgpe_slab* s, void* spec_y);
+int dgpe_slab_stage_c(dgpe_slab* s, const void* spec_recv, void* psi_x, void* psi_send);
+int dgpe_slab_stage_d(dgpe_slab* s, void* psi_y, double* norm_part);
+int dgpe_slab_stage_e(dgpe_slab* s, const void* psi_recv, void* psi_x, const double* norm_total);
+int dgpe_slab_end(dgpe_slab* s, void* psi_x);
+
 /* Thread-local description of the last error ("" if none). Never NULL. */
 const char* dgpe_last_error(void);
 

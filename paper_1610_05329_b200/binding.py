@@ -16,7 +16,11 @@ OK, ERR_ARG, ERR_CUDA, ERR_NOMEM, ERR_UNSUPPORTED, ERR_NONFINITE = 0, -1, -2, -3
 EXPORTS = ("dgpe_create", "dgpe_create_ex", "dgpe_last_error_code", "dgpe_destroy", "dgpe_set_stream", "dgpe_step", "dgpe_norm", "dgpe_chempot",
            "dgpe_energy", "dgpe_rms", "dgpe_energy_terms", "dgpe_dipolar", "dgpe_nonlinear", "dgpe_sweep",
            "dgpe_step_host", "dgpe_step_profile", "dgpe_kernel_name", "dgpe_kernel_bytes",
-           "dgpe_synchronize", "dgpe_bytes_per_step", "dgpe_launches_per_step", "dgpe_last_error")
+           "dgpe_synchronize", "dgpe_bytes_per_step", "dgpe_launches_per_step", "dgpe_last_error",
+           # one rank's stages of the slab-decomposed step (bound in sharded.py)
+           "dgpe_slab_create", "dgpe_slab_destroy", "dgpe_slab_set_stream", "dgpe_slab_elems", "dgpe_slab_begin",
+           "dgpe_slab_stage_a", "dgpe_slab_stage_b", "dgpe_slab_stage_c", "dgpe_slab_stage_d", "dgpe_slab_stage_e",
+           "dgpe_slab_end")
 
 _lib = None
 

@@ -83,6 +83,14 @@ struct dgpe_handle {
     int nzc = 0;
     double dx, dy, dz, dt, gamma, nu, lambda, g, gdd;
     long long N;
+    // Slab views (dgpe_slab, SV section 8f NEXT-3; "data distributed along NX"): nx, ny above are the LOCAL extents
+    // of the arrays this handle's kernels walk; the tables are those of the global grid gnx x gny x nz, entered at the
+    // offsets x0, y0 of the slab.  A view holds whole lines along y (has_y: an x slab) or along x (has_x: a y slab).
+    // Ordinary handles: gnx = nx, gny = ny, no offsets, both.
+    int gnx = 0, gny = 0, x0 = 0, y0 = 0;
+    bool has_x = true, has_y = true;
+    bool own_spec = true;            // false: the half-spectrum buffer is handed in per call (y-slab view)
+    double inv_ntot = 0.0;           // 1/(gnx gny nz): normalisation of the inverse transform (R#10)
     cudaStream_t stream = nullptr;
     int num_sms = 148;
     bool force_generic = false;      // DGPE_GENERIC=1: runtime-plan kernels only (A/B checks)
@@ -360,8 +368,11 @@ static int init_handle(dgpe_handle* h)
         if (o.pf_mult > 0) h->pf_mult = o.pf_mult;
     }
 
-    if ((rc = make_plan(h, nx, &h->plan_x, &h->tw_x, 128))) return rc;
-    if ((rc = make_plan(h, ny, &h->plan_y, &h->tw_y, 128))) return rc;
+    if (!h->gnx) { h->gnx = nx; h->gny = ny; }
+    const int gnx = h->gnx, gny = h->gny;
+    h->inv_ntot = 1.0 / ((double)gnx * (double)gny * (double)nz);
+    if (h->has_x && (rc = make_plan(h, nx, &h->plan_x, &h->tw_x, 128))) return rc;
+    if (h->has_y && (rc = make_plan(h, ny, &h->plan_y, &h->tw_y, 128))) return rc;
     if ((rc = make_plan(h, M, &h->plan_zh, &h->tw_zh, 64))) return rc;
     {
         std::vector<cplx> tw(M + 1);
@@ -372,9 +383,11 @@ static int init_handle(dgpe_handle* h)
         }
         if ((rc = upload(h, tw, &h->tw_split))) return rc;
     }
-    if ((rc = upload(h, wavenum_sq(nx, h->dx, nx), &h->kx2))) return rc;
-    if ((rc = upload(h, wavenum_sq(ny, h->dy, ny), &h->ky2))) return rc;
+    if ((rc = upload(h, wavenum_sq(gnx, h->dx, gnx), &h->kx2))) return rc;
+    if ((rc = upload(h, wavenum_sq(gny, h->dy, gny), &h->ky2))) return rc;
     if ((rc = upload(h, wavenum_sq(nz, h->dz, nzh), &h->kz2))) return rc;
+    h->kx2 += h->x0;      // tables of the global grid, entered at the slab's offset (the uploads stay owned at their bases)
+    h->ky2 += h->y0;
 
     auto coord_tables = [&](int n, double d, double om, double** v, double** c2) -> int {
         std::vector<double> tv(n), tc(n);
@@ -387,13 +400,16 @@ static int init_handle(dgpe_handle* h)
         if (r1) return r1;
         return upload(h, tc, c2);
     };
-    if ((rc = coord_tables(nx, h->dx, h->gamma, &h->vx, &h->x2))) return rc;
-    if ((rc = coord_tables(ny, h->dy, h->nu, &h->vy, &h->y2))) return rc;
+    if ((rc = coord_tables(gnx, h->dx, h->gamma, &h->vx, &h->x2))) return rc;
+    if ((rc = coord_tables(gny, h->dy, h->nu, &h->vy, &h->y2))) return rc;
     if ((rc = coord_tables(nz, h->dz, h->lambda, &h->vz, &h->z2))) return rc;
+    h->vx += h->x0; h->x2 += h->x0;
+    h->vy += h->y0; h->y2 += h->y0;
 
     const int ns[3] = {nx, ny, nz};
     const double ds[3] = {h->dx, h->dy, h->dz};
     for (int a = 0; a < 3; ++a) {
+        if ((a == 0 && !h->has_x) || (a == 1 && !h->has_y)) continue;      // a slab view never sweeps along its cut axis
         const double rr = h->dt / (4.0 * ds[a] * ds[a]);      // R#9
         // chunk length of the sweep recursions: 8 (or 16) unknowns per thread on the strided axes; on z
         // the warp-per-line kernel gives every lane ceil((nz-2)/32) unknowns
@@ -407,8 +423,10 @@ static int init_handle(dgpe_handle* h)
         if (rc) return rc;
     }
 
-    CU(cudaMalloc(&h->spec, sizeof(cplx) * (size_t)nx * ny * nzh));
-    h->owned.push_back(h->spec);
+    if (h->own_spec) {
+        CU(cudaMalloc(&h->spec, sizeof(cplx) * (size_t)nx * ny * nzh));
+        h->owned.push_back(h->spec);
+    }
     size_t nblk = std::max({(size_t)(((long long)ny * nz + 7) / 8), (size_t)nx * ((nz + 7) / 8),
                             (size_t)(((long long)nx * ny + 7) / 8), (size_t)4096});
     CU(cudaMalloc(&h->partials, sizeof(double) * nblk * MAX_RED));
@@ -702,7 +720,7 @@ static int launch_fft_xy_n(dgpe_handle* h, const LineMap& map, int nbatch, const
     int ctas_per_sm = 0;
     int rc = kernel_setup((const void*)kern, xy_threads<N>(), smem, &ctas_per_sm);
     if (rc) return rc;
-    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 2.0 * 3.14159265358979323846264338327950288 / ((double)h->nx * h->dx), 1.0 / (double)h->N,
+    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 2.0 * 3.14159265358979323846264338327950288 / ((double)h->nx * h->dx), h->inv_ntot,
               (h->prefetch & (KIND == FFT_X_UDD ? PF_FFT_X : PF_FFT_Y)) ? h->pf_mult * ctas_per_sm * h->num_sms : 0};
     dim3 grid((map.ncols + TILE_COLS - 1) / TILE_COLS, nbatch);
     kern<<<grid, xy_threads<N>(), smem, h->stream>>>(h->spec, map, tw, U);
@@ -834,7 +852,7 @@ static int launch_fft_tma_xudd_n(dgpe_handle* h)
     W.n = N; W.box_rows = N / nbox;
     W.tiles_per_batch = (int)((ncols + TILE_COLS - 1) / TILE_COLS);
     W.ntiles = W.tiles_per_batch;
-    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 2.0 * 3.14159265358979323846264338327950288 / ((double)h->nx * h->dx), 1.0 / (double)h->N, 0};
+    UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 2.0 * 3.14159265358979323846264338327950288 / ((double)h->nx * h->dx), h->inv_ntot, 0};
     kern<<<std::min(W.ntiles, h->num_sms), xy_threads<N>(), smem, h->stream>>>(tmap, W, h->tw_x, U, (int)ncols);
     return check_launch("k_fft_tma_xudd");
 }
@@ -906,11 +924,11 @@ static int launch_fft_x_udd(dgpe_handle* h)
     if (tx <= 512) {
         if ((rcs = kernel_setup((const void*)k_fft_x_udd<512>, tx, smx, nullptr))) return rcs;
         k_fft_x_udd<512><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
-                                                                     1.0 / (double)h->N);
+                                                                     h->inv_ntot);
     } else {
         if ((rcs = kernel_setup((const void*)k_fft_x_udd<1024>, tx, smx, nullptr))) return rcs;
         k_fft_x_udd<1024><<<(ny * nzh + 7) / 8, tx, smx, h->stream>>>(h->spec, mx, h->plan_x, nzh, h->kx2, h->ky2, h->kz2,
-                                                                      1.0 / (double)h->N);
+                                                                      h->inv_ntot);
     }
     return check_launch("k_fft_x_udd");
 }
@@ -1350,6 +1368,203 @@ extern "C" int dgpe_sweep(dgpe_handle* h, void* psi, int axis)
     { int rcd = check_device(h); if (rcd) return rcd; }
     if (axis < 0 || axis > 2) return fail(DGPE_ERR_ARG, "axis %d not in 0..2", axis);
     return launch_sweep(h, (cplx*)psi, axis, false);
+}
+
+// ------------------------------------------------------------------------------------------------
+// slab-decomposed step (SV section 8f NEXT-3): one rank's stages
+// ------------------------------------------------------------------------------------------------
+struct dgpe_slab {
+    int P = 1, rank = 0, gnx = 0, gny = 0, nz = 0, nzh = 0, nxl = 0, nyl = 0;
+    dgpe_handle* hx = nullptr;      // x slab [nxl][gny][nz]: whole lines along y and z
+    dgpe_handle* hy = nullptr;      // y slab [gnx][nyl][nz]: whole lines along x (and z)
+};
+
+static dgpe_handle* make_view(int nx, int ny, int nz, int gnx, int gny, int x0, int y0, bool has_x, bool has_y,
+                              double dx, double dy, double dz, double dt, double gamma, double nu, double lambda, double g,
+                              double gdd, int mode, bool need_spec)
+{
+    dgpe_handle* h = new (std::nothrow) dgpe_handle();
+    if (!h) { fail(DGPE_ERR_NOMEM, "host allocation failed"); return nullptr; }
+    int* f = reinterpret_cast<int*>(&h->opt);
+    for (size_t i = 0; i < sizeof(dgpe_options) / sizeof(int); ++i) f[i] = -1;
+    h->nx = nx; h->ny = ny; h->nz = nz; h->nzh = nz / 2 + 1;
+    h->gnx = gnx; h->gny = gny; h->x0 = x0; h->y0 = y0; h->has_x = has_x; h->has_y = has_y;
+    h->rpsi = false; h->mode = mode; h->nzc = nz;
+    h->dx = dx; h->dy = dy; h->dz = dz; h->dt = dt;
+    h->gamma = gamma; h->nu = nu; h->lambda = lambda; h->g = g; h->gdd = gdd;
+    h->N = (long long)nx * ny * nz;
+    h->own_spec = need_spec;
+    if (init_handle(h) != DGPE_OK) {
+        char keep[sizeof(g_err)];
+        std::memcpy(keep, g_err, sizeof(keep));
+        dgpe_destroy(h);
+        std::memcpy(g_err, keep, sizeof(keep));
+        return nullptr;
+    }
+    return h;
+}
+
+extern "C" dgpe_slab* dgpe_slab_create(int nx, int ny, int nz, double dx, double dy, double dz, double dt, double gamma,
+                                       double nu, double lambda, double g, double gdd, int mode, int nranks, int rank)
+{
+    g_err[0] = 0;
+    g_err_code = DGPE_OK;
+    auto bad = [](int code) -> dgpe_slab* { g_err_code = code; return nullptr; };
+    const int ns[3] = {nx, ny, nz};
+    for (int a = 0; a < 3; ++a) {
+        if (ns[a] < 4) return bad(fail(DGPE_ERR_ARG, "grid size %d < 4", ns[a]));
+        if (!smooth2357(ns[a])) return bad(fail(DGPE_ERR_ARG, "grid size %d is not of the form 2^a 3^b 5^c 7^d 11^e 13^f", ns[a]));
+        if (ns[a] > DGPE_MAX_N) return bad(fail(DGPE_ERR_UNSUPPORTED, "grid size %d > %d", ns[a], DGPE_MAX_N));
+    }
+    if (nz % 2) return bad(fail(DGPE_ERR_ARG, "nz = %d must be even", nz));
+    if (!(dx > 0.0) || !(dy > 0.0) || !(dz > 0.0) || !(dt > 0.0) || !std::isfinite(dx) || !std::isfinite(dy) ||
+        !std::isfinite(dz) || !std::isfinite(dt))
+        return bad(fail(DGPE_ERR_ARG, "dx, dy, dz, dt must be positive and finite"));
+    if (mode != DGPE_IMAG && mode != DGPE_REAL) return bad(fail(DGPE_ERR_ARG, "mode %d is neither DGPE_IMAG nor DGPE_REAL", mode));
+    // "NX and NY must be divisible by the number of processes ... programs will test ... and inform the user"
+    if (nranks < 1 || rank < 0 || rank >= nranks) return bad(fail(DGPE_ERR_ARG, "rank %d of %d ranks", rank, nranks));
+    if (nx % nranks || ny % nranks)
+        return bad(fail(DGPE_ERR_ARG, "nx = %d and ny = %d must both be divisible by the number of ranks %d", nx, ny, nranks));
+    dgpe_slab* s = new (std::nothrow) dgpe_slab();
+    if (!s) return bad(fail(DGPE_ERR_NOMEM, "host allocation failed"));
+    s->P = nranks; s->rank = rank; s->gnx = nx; s->gny = ny; s->nz = nz; s->nzh = nz / 2 + 1;
+    s->nxl = nx / nranks; s->nyl = ny / nranks;
+    s->hx = make_view(s->nxl, ny, nz, nx, ny, rank * s->nxl, 0, false, true, dx, dy, dz, dt, gamma, nu, lambda, g, gdd, mode, true);
+    if (s->hx) s->hy = make_view(nx, s->nyl, nz, nx, ny, 0, rank * s->nyl, true, false, dx, dy, dz, dt, gamma, nu, lambda, g, gdd, mode, false);
+    if (!s->hx || !s->hy) {
+        char keep[sizeof(g_err)];
+        std::memcpy(keep, g_err, sizeof(keep));
+        dgpe_slab_destroy(s);
+        std::memcpy(g_err, keep, sizeof(keep));
+        return bad(DGPE_ERR_CUDA);
+    }
+    return s;
+}
+
+extern "C" void dgpe_slab_destroy(dgpe_slab* s)
+{
+    if (!s) return;
+    dgpe_destroy(s->hx);
+    dgpe_destroy(s->hy);
+    delete s;
+}
+
+extern "C" int dgpe_slab_set_stream(dgpe_slab* s, void* cuda_stream)
+{
+    if (!s) return fail(DGPE_ERR_ARG, "NULL slab");
+    s->hx->stream = s->hy->stream = (cudaStream_t)cuda_stream;
+    return DGPE_OK;
+}
+
+extern "C" long long dgpe_slab_elems(const dgpe_slab* s, int spectrum)
+{
+    if (!s) return 0;
+    return (long long)s->nxl * s->gny * (spectrum ? s->nzh : s->nz);
+}
+
+// block (q) of the slab array [nxl][gny][w] that belongs to rank q's y range, to / from a buffer [P][nxl][nyl][w]
+// (the exchanged blocks are (NX/P) x (NY/P) x NZ each: P:L59; the strided side is what the paper's CUDA/MPI package maps
+// with an MPI derived datatype, here one strided copy per peer)
+static int slab_pack(const dgpe_slab* s, cudaStream_t st, const cplx* slab, cplx* buf, int w, bool unpack)
+{
+    const size_t width = (size_t)s->nyl * w * sizeof(cplx), pitch = (size_t)s->gny * w * sizeof(cplx);
+    for (int q = 0; q < s->P; ++q) {
+        const cplx* a = slab + (size_t)q * s->nyl * w;
+        cplx* b = buf + (size_t)q * s->nxl * s->nyl * w;
+        if (unpack) CU(cudaMemcpy2DAsync(const_cast<cplx*>(a), pitch, b, width, width, s->nxl, cudaMemcpyDeviceToDevice, st));
+        else CU(cudaMemcpy2DAsync(b, width, a, pitch, width, s->nxl, cudaMemcpyDeviceToDevice, st));
+    }
+    return DGPE_OK;
+}
+
+extern "C" int dgpe_slab_begin(dgpe_slab* s)
+{
+    if (!s) return fail(DGPE_ERR_ARG, "NULL slab");
+    int rc = check_device(s->hx);
+    if (rc) return rc;
+    if ((rc = set_scal(s->hx, 1))) return rc;
+    return set_scal(s->hy, 1);
+}
+
+// a: density + R2C along z (K1) and FFT along y (K2) on the x slab; the half-spectrum leaves in blocks per peer
+extern "C" int dgpe_slab_stage_a(dgpe_slab* s, const void* psi_x, void* spec_send)
+{
+    if (!s || !psi_x || !spec_send) return fail(DGPE_ERR_ARG, "NULL argument");
+    int rc;
+    if ((rc = launch_k1(s->hx, (const cplx*)psi_x))) return rc;
+    if ((rc = launch_fft_y(s->hx, false))) return rc;
+    return slab_pack(s, s->hx->stream, s->hx->spec, (cplx*)spec_send, s->nzh, false);
+}
+
+// b: FFT along x, Udd~(k)/N, inverse FFT along x (K3) in place on the y slab [nx][nyl][nzh] the exchange delivered
+extern "C" int dgpe_slab_stage_b(dgpe_slab* s, void* spec_y)
+{
+    if (!s || !spec_y) return fail(DGPE_ERR_ARG, "NULL argument");
+    cplx* own = s->hy->spec;
+    s->hy->spec = (cplx*)spec_y;
+    const int rc = launch_fft_x_udd(s->hy);
+    s->hy->spec = own;
+    return rc;
+}
+
+// c: the half-spectrum is back on the x slab: inverse FFT along y (K4), C2R along z + nonlinear exponential (K5),
+//    sweeps along z and y; psi leaves in blocks per peer
+extern "C" int dgpe_slab_stage_c(dgpe_slab* s, const void* spec_recv, void* psi_x, void* psi_send)
+{
+    if (!s || !spec_recv || !psi_x || !psi_send) return fail(DGPE_ERR_ARG, "NULL argument");
+    dgpe_handle* h = s->hx;
+    int rc;
+    if ((rc = slab_pack(s, h->stream, h->spec, const_cast<cplx*>((const cplx*)spec_recv), s->nzh, true))) return rc;
+    if ((rc = launch_fft_y(h, true))) return rc;
+    if (h->zfast) {
+        if ((rc = launch_z_main(h, (cplx*)psi_x, 1, nullptr))) return rc;
+    } else {
+        if ((rc = launch_c2r(h, (cplx*)psi_x, h->mode == DGPE_IMAG ? 0 : 1, nullptr))) return rc;
+        if ((rc = launch_sweep(h, (cplx*)psi_x, 2, false))) return rc;
+    }
+    if ((rc = launch_sweep(h, (cplx*)psi_x, 1, false))) return rc;
+    return slab_pack(s, h->stream, (const cplx*)psi_x, (cplx*)psi_send, s->nz, false);
+}
+
+// d: sweep along x in place on the y slab [nx][nyl][nz]; imaginary time: norm_part (DEVICE) <- this rank's sum |psi|^2 dV
+extern "C" int dgpe_slab_stage_d(dgpe_slab* s, void* psi_y, double* norm_part)
+{
+    if (!s || !psi_y) return fail(DGPE_ERR_ARG, "NULL argument");
+    dgpe_handle* h = s->hy;
+    const bool imag = h->mode == DGPE_IMAG;
+    if (imag && !norm_part) return fail(DGPE_ERR_ARG, "imaginary time needs norm_part");
+    int rc;
+    if ((rc = launch_sweep(h, (cplx*)psi_y, 0, imag))) return rc;
+    if (imag) CU(cudaMemcpyAsync(norm_part, h->scal + SC_NORM, sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+    return DGPE_OK;
+}
+
+// e: psi is back on the x slab; imaginary time: norm_total (DEVICE) = the sum of all ranks' norm_part -> the scale
+//    factors of the next step's kernels
+extern "C" int dgpe_slab_stage_e(dgpe_slab* s, const void* psi_recv, void* psi_x, const double* norm_total)
+{
+    if (!s || !psi_recv || !psi_x) return fail(DGPE_ERR_ARG, "NULL argument");
+    dgpe_handle* h = s->hx;
+    int rc;
+    if ((rc = slab_pack(s, h->stream, (const cplx*)psi_x, const_cast<cplx*>((const cplx*)psi_recv), s->nz, true))) return rc;
+    if (h->mode == DGPE_IMAG) {
+        if (!norm_total) return fail(DGPE_ERR_ARG, "imaginary time needs norm_total");
+        k_set_norm<<<1, 1, 0, h->stream>>>(h->scal, norm_total);
+        if ((rc = check_launch("k_set_norm"))) return rc;
+    }
+    return DGPE_OK;
+}
+
+// end of a call of nsteps steps: imaginary time -> explicit rescale to unit norm, status of the norms seen
+extern "C" int dgpe_slab_end(dgpe_slab* s, void* psi_x)
+{
+    if (!s || !psi_x) return fail(DGPE_ERR_ARG, "NULL argument");
+    dgpe_handle* h = s->hx;
+    if (h->mode != DGPE_IMAG) { CU(cudaStreamSynchronize(h->stream)); return DGPE_OK; }
+    int rc;
+    if ((rc = finish_steps(h, (cplx*)psi_x))) return rc;
+    CU(cudaStreamSynchronize(h->stream));
+    return check_finite(h);
 }
 
 // ------------------------------------------------------------------------------------------------

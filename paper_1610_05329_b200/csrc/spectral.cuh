@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_fft_x_udd(cplx* __restrict__ spec, 
         for (int i = b; i < n; i += (blockDim.x >> 3)) {
             const double k2 = __ldg(&kx2[i]) + qy + qz;
             double u = 0.0;
-            if (i != 0 || ky != 0 || kz != 0) u = FOUR_PI_3 * (3.0 * qz / k2 - 1.0);
+            if (k2 != 0.0) u = FOUR_PI_3 * (3.0 * qz / k2 - 1.0);      // k2 is exactly zero only at the origin (R#11)
             u *= invN;
             cplx v = sm[i * TILE_COLS + c];
             sm[i * TILE_COLS + c] = mk(v.x * u, v.y * u);

@@ -214,4 +214,15 @@ __global__ void k_set_scal(double* scal, double s2, double s1, int clear_bad)
     if (clear_bad) scal[SC_BAD] = 0.0;
 }
 
+// scal <- the scale factors of a norm that was summed over the ranks of a slab decomposition (dgpe_slab): the
+// folded reduction of the last sweep only knows its own slab's part
+__global__ void k_set_norm(double* scal, const double* __restrict__ norm_total)
+{
+    const double norm = *norm_total;
+    scal[SC_NORM] = norm;
+    scal[SC_S2] = 1.0 / norm;
+    scal[SC_S1] = 1.0 / sqrt(norm);
+    if (!(norm > 0.0) || !isfinite(norm)) scal[SC_BAD] = 1.0;
+}
+
 }  // namespace dgpe

@@ -83,7 +83,6 @@ k_fft_xy(cplx* __restrict__ data, LineMap map, const cplx* __restrict__ tw, UddA
         // ky^2, kz^2 of this thread's column, loaded now and used after the forward passes
         const int ky = (colok ? col : 0) / U.nzh, kz = (colok ? col : 0) - ky * U.nzh;
         const double qy = __ldg(&U.ky2[ky]), qz = __ldg(&U.kz2[kz]);
-        const bool origin_col = (ky == 0 && kz == 0);
         // forward passes 0 .. L-2 through the tile
         ct_fft_range<N, false, false, NBF, SyncCta, PosTile, 0, L - 1, true>(colsm, b, on, tw, from_g, to_g);
         // last forward pass, Udd~(k)/N, first inverse pass: one set of registers
@@ -113,7 +112,7 @@ k_fft_xy(cplx* __restrict__ data, LineMap map, const cplx* __restrict__ tw, UddA
                 rk = rk * (2.0 - k2 * rk);
                 rk = rk * (2.0 - k2 * rk);
                 double u = FOUR_PI_3 * (3.0 * qz * rk - 1.0);
-                if (origin_col && idx == 0) u = 0.0;
+                if (k2 == 0.0) u = 0.0;      // Udd~(0) = 0 (R#11); k2 is exactly zero only at the origin
                 u *= U.invN;
                 return mk(v.x * u, v.y * u);
             });

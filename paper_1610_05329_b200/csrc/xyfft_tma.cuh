@@ -140,7 +140,6 @@ k_fft_tma_xudd(const __grid_constant__ CUtensorMap tmap, TmaWalk W, const cplx* 
         const int cidx = min((first + it * stride) * TILE_COLS + c, ncols - 1);
         const int ky = cidx / U.nzh, kz = cidx - ky * U.nzh;
         const double qy = __ldg(&U.ky2[ky]), qz = __ldg(&U.kz2[kz]);
-        const bool origin_col = (ky == 0 && kz == 0);
         mbar_wait(&full[st], (unsigned)((it / NSTAGE) & 1));
 
         // forward pass 0 by hand, so that the refill of the stage tile it-1 used can be issued after its barrier
@@ -184,7 +183,7 @@ k_fft_tma_xudd(const __grid_constant__ CUtensorMap tmap, TmaWalk W, const cplx* 
                 rk = rk * (2.0 - k2 * rk);
                 rk = rk * (2.0 - k2 * rk);
                 double u = FOUR_PI_3 * (3.0 * qz * rk - 1.0);
-                if (origin_col && idx == 0) u = 0.0;
+                if (k2 == 0.0) u = 0.0;      // Udd~(0) = 0 (R#11); k2 is exactly zero only at the origin
                 u *= U.invN;
                 return mk(v.x * u, v.y * u);
             });

@@ -306,19 +306,29 @@ def test_real_time_phase_range_of_the_fast_sincos(gpu, oracle, shape, theta_max)
     assert abs(G.norm(t) / O.norm(a) - 1.0) <= 1e-12               # |exp(-i theta)| = 1 whatever theta
 
 
-def test_real_time_non_finite_phase_gives_nan_like_libm(gpu, oracle):
+def test_real_time_huge_and_non_finite_phases(gpu, oracle):
+    """One point with a phase of 5e299 rad: far beyond the fast reduction, so the kernel must have taken the library
+    routine there -- its result is still a pure rotation (|psi'| = |psi| to rounding; the fast reduction would return
+    garbage) -- while every other point of the field keeps its 1e-12 parity.  And an overflowing density (inf) gives
+    NaN on both sides, as sin(inf) does."""
     shape = (8, 8, 64)
     args = (*shape, 0.3, 0.25, 0.2, 0.01, 1.0, 0.7, 1.3, 50.0, 0.0, 1)
     psi = inputs.random_state(shape, 42)
-    psi[3, 4, 20] = 1e200                                          # |psi|^2 overflows: theta = inf, sin(inf) = NaN
+    psi[3, 4, 20] = 1e150
     G, O = gpu.Dgpe(*args), oracle.Oracle(*args)
     t, a = dev(psi), psi.copy()
     G.nonlinear(t)
     O.nonlinear(a)
     got = t.cpu().numpy()
-    assert np.array_equal(np.isnan(got.real) | np.isnan(got.imag), np.isnan(a.real) | np.isnan(a.imag))
-    ok = ~(np.isnan(a.real) | np.isnan(a.imag))
-    assert np.max(np.abs(got[ok] - a[ok])) <= 1e-12 and (~ok).sum() >= 1
+    assert abs(abs(got[3, 4, 20]) / 1e150 - 1.0) <= 1e-14 and abs(abs(a[3, 4, 20]) / 1e150 - 1.0) <= 1e-14
+    got[3, 4, 20] = a[3, 4, 20] = 0.0
+    assert np.max(np.abs(got - a)) <= 1e-12
+    psi[3, 4, 20] = 1e200                                           # |psi|^2 = inf: theta = inf
+    t, a = dev(psi), psi.copy()
+    G.nonlinear(t)
+    O.nonlinear(a)
+    got = t.cpu().numpy()
+    assert np.isnan(got[3, 4, 20].real) and np.isnan(a[3, 4, 20].real)
 
 
 def test_handles_of_different_sizes_alive_together(gpu, oracle):
