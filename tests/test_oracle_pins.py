@@ -481,6 +481,29 @@ def test_p13_c2_noisefree_first_step(oracle):
 # argument checking
 # ------------------------------------------------------------------------------------------
 
+def test_nonfinite_norm_status_and_no_clamp(oracle):
+    """R#18 / SURVEY 8(b): the imaginary-time renormalisation has no clamp.  A zero state has norm 0 (psi / sqrt(0)), an
+    overflowing exponential gives inf: both must come back as ODGPE_ERR_NONFINITE, the status the CUDA path is compared
+    with for the literal 200-step C4 call; a healthy state returns OK, and real time never reports it (no norm taken)."""
+    shape = (8, 8, 8)
+    phys = (0.5, 0.5, 0.5, 0.01, 1.0, 1.0, 1.0, 1.0, 1.0)
+    Oi, Or = oracle.Oracle(*shape, *phys, 0), oracle.Oracle(*shape, *phys, 1)
+    good = inputs.random_state(shape, 61) * 0.3
+    assert Oi.step(good.copy(), 2) == oracle.OK
+    zero = np.zeros(shape, dtype=np.complex128)
+    assert Oi.step(zero, 1) == oracle.ERR_NONFINITE                   # norm = 0
+    assert Or.step(np.zeros(shape, dtype=np.complex128), 1) == oracle.OK
+    # exp(-dt H) with H = g |psi|^2 hugely negative (attractive contact term): overflow -> inf norm
+    Oneg = oracle.Oracle(*shape, 0.5, 0.5, 0.5, 0.01, 1.0, 1.0, 1.0, -1.0e6, 0.0, 0)
+    big = inputs.random_state(shape, 62) * 30.0
+    a = big.copy()
+    assert Oneg.step(a, 1) == oracle.ERR_NONFINITE
+    assert not np.all(np.isfinite(a.view(np.float64)))                # nothing was clamped
+    # the status is sticky within a call: a later finite norm does not clear it
+    b = zero.copy()
+    assert Oi.step(b, 3) == oracle.ERR_NONFINITE
+
+
 def test_create_rejects_bad_arguments(oracle):
     good = list(inputs.CONFIGS["C1"].create_args())
     for pos, bad in [(0, 3), (3, 0.0), (4, -1.0), (6, 0.0), (12, 2)]:
