@@ -25,7 +25,9 @@ k_fft_tma(const __grid_constant__ CUtensorMap tmap, TmaWalk W, const cplx* __res
     static_assert(L >= 2, "the pipelined kernel is for the long lines");
     extern __shared__ unsigned char smem_dyn[];
     __shared__ __align__(8) unsigned long long full[NSTAGE];
-    cplx* stages = reinterpret_cast<cplx*>((reinterpret_cast<uintptr_t>(smem_dyn) + 127) & ~uintptr_t(127));
+    // 128-byte aligned start of the stages, as an OFFSET into the shared array: the pointer keeps its address space, so
+    // the tile accesses compile to LDS/STS (through a round trip over an integer they were generic LD.E/ST.E)
+    cplx* stages = reinterpret_cast<cplx*>(smem_dyn + ((128u - (smem_addr(smem_dyn) & 127u)) & 127u));
     constexpr int tile_elems = N * TILE_COLS;
     constexpr unsigned tile_bytes = (unsigned)tile_elems * 16u;
     const int tid = threadIdx.x, c = tid & 7, b = tid >> 3;
@@ -105,7 +107,9 @@ k_fft_tma_xudd(const __grid_constant__ CUtensorMap tmap, TmaWalk W, const cplx* 
     static_assert(L >= 2, "the pipelined kernel is for the long lines");
     extern __shared__ unsigned char smem_dyn[];
     __shared__ __align__(8) unsigned long long full[NSTAGE];
-    cplx* stages = reinterpret_cast<cplx*>((reinterpret_cast<uintptr_t>(smem_dyn) + 127) & ~uintptr_t(127));
+    // 128-byte aligned start of the stages, as an OFFSET into the shared array: the pointer keeps its address space, so
+    // the tile accesses compile to LDS/STS (through a round trip over an integer they were generic LD.E/ST.E)
+    cplx* stages = reinterpret_cast<cplx*>(smem_dyn + ((128u - (smem_addr(smem_dyn) & 127u)) & 127u));
     constexpr int tile_elems = N * TILE_COLS;
     constexpr unsigned tile_bytes = (unsigned)tile_elems * 16u;
     const int tid = threadIdx.x, c = tid & 7, b = tid >> 3;

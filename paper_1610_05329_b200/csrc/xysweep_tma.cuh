@@ -41,7 +41,9 @@ k_sweep_tma(const __grid_constant__ CUtensorMap tmap, TmaWalk W, SweepTables<CT>
     __shared__ cplx smX[NTMAX / 8][TILE_COLS];
     __shared__ double red[32];
     __shared__ __align__(8) unsigned long long full[NSTAGE];
-    cplx* stages = reinterpret_cast<cplx*>((reinterpret_cast<uintptr_t>(smem_dyn) + 127) & ~uintptr_t(127));
+    // 128-byte aligned start of the stages, as an OFFSET into the shared array: the pointer keeps its address space, so
+    // the tile accesses compile to LDS/STS (through a round trip over an integer they were generic LD.E/ST.E)
+    cplx* stages = reinterpret_cast<cplx*>(smem_dyn + ((128u - (smem_addr(smem_dyn) & 127u)) & 127u));
     const int n = W.n;
     const int tile_elems = n * TILE_COLS;
     const unsigned tile_bytes = (unsigned)tile_elems * 16u;
