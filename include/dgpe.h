@@ -51,8 +51,8 @@ typedef struct dgpe_handle dgpe_handle;
  * nx*ny*nz plain DOUBLES (8 bytes per point, same row-major layout, 16-byte aligned) and the step moves
  * 72N + 8S bytes instead of 144N + 8S.  The results equal those of DGPE_IMAG on the same psi with a zero
  * imaginary part.  nz must be one of the specialised z lengths (64, 128, 160, 192, 240, 250, 256, 320, 384,
- * 480, 500, 512, 640, 768), else dgpe_create fails with DGPE_ERR_UNSUPPORTED.  The observables copy psi into
- * a complex array the handle owns (16*nx*ny*nz bytes, allocated on first use).
+ * 480, 500, 512, 640, 768), else dgpe_create fails with DGPE_ERR_UNSUPPORTED.  The observables take the same
+ * doubles (their kernels are templated on the element type).
  */
 enum { DGPE_IMAG = 0, DGPE_REAL = 1, DGPE_IMAG_RPSI = 2 };
 
