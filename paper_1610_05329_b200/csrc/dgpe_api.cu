@@ -627,7 +627,7 @@ static int launch_z_main_c(dgpe_handle* h, cplx* psi, double* phi_out)
     T.r = to_ct<CT>(S.r);
     T.omr2 = to_ct<CT>(1.0 - 2.0 * S.r);
     T.inv = (const CT*)S.inv; T.cc = (const CT*)S.cc; T.F = (const CT*)S.F; T.Gm = (const CT*)S.Gm;
-    T.Ach = (const CT*)S.Ach; T.Bch = (const CT*)S.Bch;
+    T.Ach = (const CT*)S.Ach; T.Bch = (const CT*)S.Bch; T.ztab = (const CT*)S.ztab;
     T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb; T.gU = S.gU;
     if (SWEEP && (S.Lc != LC || S.G > ZGeom<NZ>::T)) return fail(DGPE_ERR_CUDA, "z sweep tables do not match the z-line kernel");
     ChunkTabs<CT, LC> P;
@@ -1059,7 +1059,7 @@ static int launch_sweep_t(dgpe_handle* h, cplx* psi, int axis, bool fold)
     T.r = to_ct<CT>(S.r);
     T.omr2 = to_ct<CT>(1.0 - 2.0 * S.r);
     T.inv = (const CT*)S.inv; T.cc = (const CT*)S.cc; T.F = (const CT*)S.F; T.Gm = (const CT*)S.Gm;
-    T.Ach = (const CT*)S.Ach; T.Bch = (const CT*)S.Bch;
+    T.Ach = (const CT*)S.Ach; T.Bch = (const CT*)S.Bch; T.ztab = (const CT*)S.ztab;
     T.Lc = S.Lc; T.G = S.G; T.Kf = S.Kf; T.Kb = S.Kb; T.gU = S.gU;
     SweepFold F;
     F.enabled = fold ? 1 : 0;

@@ -42,6 +42,7 @@ struct SweepTables {
     const CT* Gm;      // [n]   backward running product inside the chunk
     const CT* Ach;     // [G]   chunk forward factor
     const CT* Bch;     // [G]   chunk backward factor
+    const CT* ztab;    // [8 Lc] compact table for CONSTTAB kernels: [inv, c, F, G] of chunk 0, then of the converged chunk
     int Lc, G, Kf, Kb;
     int gU;            // chunks gU .. G-2 have bit-identical table entries (G if none): a lane-per-chunk kernel
                        // may read chunk gU's entries for all of them (one broadcast address)

@@ -50,6 +50,8 @@ k_sweep_xy(cplx* __restrict__ psi, LineMap map, SweepTables<CT> T, SweepFold fol
                 prefetch_l2(psi + (long long)by * map.batch_stride + (long long)bx * TILE_COLS * map.col_stride + (long long)j * es);
     }
     const bool g0 = g == 0;
+    // (kernel parameters here: read through L1 instead, as the TMA sweep and the z kernels do, this kernel -- whose loads
+    // already wait on memory -- got slower: 512^3 x sweep 0.82 -> 1.09 ms)
     auto t_inv = [&](int i) { if constexpr (CONSTTAB) return g0 ? P.inv0[i] : P.invU[i]; else return __ldg(&T.inv[s + i]); };
     auto t_cc = [&](int i) { if constexpr (CONSTTAB) return g0 ? P.cc0[i] : P.ccU[i]; else return __ldg(&T.cc[s + i]); };
     auto t_F = [&](int i) { if constexpr (CONSTTAB) return P.fU[i]; else return __ldg(&T.F[s + i]); };
