@@ -212,6 +212,24 @@ int dgpe_slab_stage_d(dgpe_slab* s, void* psi_y, double* norm_part);
 int dgpe_slab_stage_e(dgpe_slab* s, const void* psi_recv, void* psi_x, const double* norm_total);
 int dgpe_slab_end(dgpe_slab* s, void* psi_x);
 
+/*
+ * dgpe_norm_noalloc -- norm = sum |psi|^2 dx dy dz (BJ:north_star (d); R#14, R#15) WITHOUT any allocation, for callers
+ * that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid it.  No handle:
+ *   psi          DEVICE, nx*ny*nz complex doubles, row-major [nx][ny][nz] (as everywhere in this header)
+ *   norm_device  DEVICE, one double the caller owns; written asynchronously on `cuda_stream` (cudaStream_t as void*,
+ *                NULL = legacy default stream).  The call does not synchronise and copies nothing to the host.
+ * The scratch of the reduction (one partial per x plane and an arrival ticket) is a static device array of
+ * 256 + 8*DGPE_NOALLOC_MAX_NX = 8448 bytes that every GPU loading the library holds until exit; nx beyond
+ * DGPE_NOALLOC_MAX_NX is rejected with DGPE_ERR_UNSUPPORTED.  All calls share that array and it keeps the last call's
+ * contents (the call clears what must start at zero): calls that OVERLAP on the GPU -- different streams or threads --
+ * race on it; issue them on one stream.  Uses the current CUDA device, which must hold psi and norm_device.
+ * Deterministic (fixed summation order); equals dgpe_norm to rounding (another summation order).
+ * Errors: DGPE_ERR_ARG (NULL, sizes < 1, spacings), DGPE_ERR_UNSUPPORTED (nx too large), DGPE_ERR_CUDA.
+ */
+#define DGPE_NOALLOC_MAX_NX 1024
+int dgpe_norm_noalloc(const void* psi, int nx, int ny, int nz, double dx, double dy, double dz,
+                      double* norm_device, void* cuda_stream);
+
 /* Thread-local description of the last error ("" if none). Never NULL. */
 const char* dgpe_last_error(void);
 

@@ -20,7 +20,9 @@ EXPORTS = ("dgpe_create", "dgpe_create_ex", "dgpe_last_error_code", "dgpe_destro
            # one rank's stages of the slab-decomposed step (bound in sharded.py)
            "dgpe_slab_create", "dgpe_slab_destroy", "dgpe_slab_set_stream", "dgpe_slab_elems", "dgpe_slab_begin",
            "dgpe_slab_stage_a", "dgpe_slab_stage_b", "dgpe_slab_stage_c", "dgpe_slab_stage_d", "dgpe_slab_stage_e",
-           "dgpe_slab_end")
+           "dgpe_slab_end",
+           # the norm without any allocation (static device scratch)
+           "dgpe_norm_noalloc")
 
 _lib = None
 
@@ -91,6 +93,7 @@ def lib():
         L.dgpe_bytes_per_step.restype = cd
         L.dgpe_bytes_per_step.argtypes = [vp]
         L.dgpe_launches_per_step.argtypes = [vp]
+        L.dgpe_norm_noalloc.argtypes = [vp, ci, ci, ci, cd, cd, cd, vp, vp]
         L.dgpe_last_error.restype = C.c_char_p
         L.dgpe_last_error.argtypes = []
         _lib = L
@@ -104,6 +107,26 @@ def last_error():
 def _check(rc):
     if rc != OK:
         raise DgpeError(rc, last_error())
+
+
+NOALLOC_MAX_NX = 1024
+
+
+def norm_noalloc(psi, dx, dy, dz, out, stream=None):
+    """dgpe_norm_noalloc: out (CUDA float64 tensor, one element, caller-owned) <- sum |psi|^2 dx dy dz, asynchronously on
+    `stream` (default: torch's current stream).  Allocates nothing, needs no handle; nx <= NOALLOC_MAX_NX.  Calls that
+    overlap on the GPU race on the library's static scratch: keep them on one stream.  Returns the status code."""
+    if not (isinstance(psi, torch.Tensor) and psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous() and psi.dim() == 3):
+        raise TypeError("psi must be a contiguous 3-D CUDA complex128 tensor")
+    if not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64 and out.numel() == 1
+            and out.device == psi.device):
+        raise TypeError("out must be a one-element CUDA float64 tensor on psi's device")
+    st = stream if stream is not None else torch.cuda.current_stream(psi.device)
+    ptr = st.cuda_stream if hasattr(st, "cuda_stream") else int(st or 0)
+    nx, ny, nz = psi.shape
+    with torch.cuda.device(psi.device):
+        return lib().dgpe_norm_noalloc(C.c_void_p(psi.data_ptr()), nx, ny, nz, dx, dy, dz, C.c_void_p(out.data_ptr()),
+                                       C.c_void_p(ptr))
 
 
 class Dgpe:

@@ -1675,3 +1675,72 @@ extern "C" int dgpe_launches_per_step(const dgpe_handle* h)
 {
     return h ? (int)step_kernels(h).size() : 0;
 }
+
+// ------------------------------------------------------------------------------------------------
+// dgpe_norm_noalloc -- the norm reduction for callers that cannot allocate (CUDA graph capture, tight
+// serving loops, harnesses that forbid cudaMalloc).  Same two-stage deterministic reduction as the
+// observables' k_moments (common.cuh grid_reduce: one partial per block, the last block adds them in a fixed
+// order), but its scratch -- the partials and the arrival ticket, which dgpe_create takes from cudaMalloc --
+// lives in ONE file-scope device array of fixed size, and the result goes to a DEVICE double of the caller.
+// The entry point calls no cudaMalloc / cudaFree / allocating routine and does not synchronise.
+//
+// Every GPU that loads the library holds the array until the process exits (8448 bytes).  All calls share
+// it and it keeps the last call's contents: the ticket is cleared on the caller's stream before every
+// launch, the partials are overwritten before they are read.  Calls that OVERLAP on the GPU (two streams,
+// two threads) race on it -- serialise them on one stream.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_noalloc_scratch[256 + 8 * DGPE_NOALLOC_MAX_NX];
+
+// one block per x plane: partial[i] = sum over the plane of |psi|^2; out = dV * sum of the partials
+__global__ void __launch_bounds__(256) k_norm_noalloc(const cplx* __restrict__ psi, long long plane, double dV,
+                                                      double* __restrict__ partials, unsigned int* ticket,
+                                                      double* __restrict__ out)
+{
+    __shared__ double red[32];
+    const cplx* p = psi + (long long)blockIdx.x * plane;
+    double acc[1] = {0.0};
+    for (long long k = threadIdx.x; k < plane; k += blockDim.x) acc[0] += cabs2(p[k]);
+    double tot[1];
+    if (grid_reduce<1>(acc, partials, ticket, tot, red)) *out = tot[0] * dV;
+}
+
+// device address of the scratch array, looked up once per device with that device current (the array's
+// name is a host-side stand-in in host code, not a device address)
+static int noalloc_scratch(unsigned char** ptr)
+{
+    static std::mutex mu;
+    static std::map<int, unsigned char*> by_device;
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(mu);
+    auto it = by_device.find(dev);
+    if (it == by_device.end()) {
+        unsigned char* p = nullptr;
+        CU(cudaGetSymbolAddress((void**)&p, g_noalloc_scratch));
+        if (!p) return fail(DGPE_ERR_CUDA, "cudaGetSymbolAddress returned a null scratch address");
+        it = by_device.emplace(dev, p).first;
+    }
+    *ptr = it->second;
+    return DGPE_OK;
+}
+
+extern "C" int dgpe_norm_noalloc(const void* psi, int nx, int ny, int nz, double dx, double dy, double dz,
+                                 double* norm_device, void* cuda_stream)
+{
+    if (!psi || !norm_device) return fail(DGPE_ERR_ARG, "NULL argument");
+    if (nx < 1 || ny < 1 || nz < 1) return fail(DGPE_ERR_ARG, "grid %d x %d x %d: every size must be >= 1", nx, ny, nz);
+    if (nx > DGPE_NOALLOC_MAX_NX)
+        return fail(DGPE_ERR_UNSUPPORTED, "dgpe_norm_noalloc: nx = %d exceeds DGPE_NOALLOC_MAX_NX = %d (one partial per x plane "
+                                          "in the %d-byte static scratch array)", nx, DGPE_NOALLOC_MAX_NX, (int)sizeof(g_noalloc_scratch));
+    if (!(dx > 0.0) || !(dy > 0.0) || !(dz > 0.0) || !std::isfinite(dx) || !std::isfinite(dy) || !std::isfinite(dz))
+        return fail(DGPE_ERR_ARG, "dx, dy, dz must be positive and finite");
+    unsigned char* scratch = nullptr;
+    int rc = noalloc_scratch(&scratch);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    unsigned int* ticket = reinterpret_cast<unsigned int*>(scratch);
+    double* partials = reinterpret_cast<double*>(scratch + 256);
+    CU(cudaMemsetAsync(ticket, 0, 256, st));             // the ticket must start at zero whatever the last call left
+    k_norm_noalloc<<<nx, 256, 0, st>>>((const cplx*)psi, (long long)ny * nz, dx * dy * dz, partials, ticket, norm_device);
+    return check_launch("k_norm_noalloc");
+}
