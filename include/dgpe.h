@@ -96,7 +96,9 @@ typedef struct dgpe_options {
     int prefetch;     /* mask of kernel families with the L2 prefetch of the next residency:
                          1 z lines, 2 y sweep, 4 x sweep, 8 y FFT, 16 x FFT                                 */
     int pf_mult;      /* prefetch distance in units of one residency (default 1)                            */
-    int reserved[9];  /* set to -1 */
+    int tma_pair;     /* 0 | 1: never | always run K2, K3, K4 at nx, ny = 512 as k_fft_pair (two tiles per SM in different
+                         phases on the TMA pipeline); default: K3 only                                        */
+    int reserved[8];  /* set to -1 */
 } dgpe_options;
 dgpe_handle* dgpe_create_ex(int nx, int ny, int nz, double dx, double dy, double dz, double dt,
                             double gamma, double nu, double lambda, double g, double gdd, int mode,

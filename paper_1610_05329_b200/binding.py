@@ -27,17 +27,17 @@ EXPORTS = ("dgpe_create", "dgpe_create_ex", "dgpe_last_error_code", "dgpe_destro
 _lib = None
 
 # fields of dgpe_options (include/dgpe.h), in order; -1 = the library's default
-OPTION_FIELDS = ("generic", "tma", "tma_fft", "tma_k3", "graph", "prefetch", "pf_mult")
+OPTION_FIELDS = ("generic", "tma", "tma_fft", "tma_k3", "graph", "prefetch", "pf_mult", "tma_pair")
 
 
 class DgpeOptions(C.Structure):
-    _fields_ = [(name, C.c_int) for name in OPTION_FIELDS] + [("reserved", C.c_int * 9)]
+    _fields_ = [(name, C.c_int) for name in OPTION_FIELDS] + [("reserved", C.c_int * 8)]
 
     def __init__(self, **kw):
         super().__init__()
         for name in OPTION_FIELDS:
             setattr(self, name, -1)
-        for i in range(9):
+        for i in range(8):
             self.reserved[i] = -1
         for name, val in kw.items():
             if name not in OPTION_FIELDS:

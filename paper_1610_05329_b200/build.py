@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdgpe.so")
 SOURCES = ["dgpe_api.cu"]
-DEPS = ["dgpe_api.cu", "common.cuh", "fft.cuh", "ctfft.cuh", "xyfft.cuh", "xysweep.cuh", "xysweep_tma.cuh", "xyfft_tma.cuh", "tma.cuh", "zline.cuh", "spectral.cuh", "sweep.cuh", "observe.cuh"]
+DEPS = ["dgpe_api.cu", "common.cuh", "fft.cuh", "ctfft.cuh", "xyfft.cuh", "xysweep.cuh", "xysweep_tma.cuh", "xyfft_tma.cuh", "xyfft_pair.cuh", "tma.cuh", "zline.cuh", "spectral.cuh", "sweep.cuh", "observe.cuh"]
 HEADER = os.path.join(os.path.dirname(HERE), "include", "dgpe.h")
 
 # (no -split-compile: measured on the B200, the kernels it produces are slower -- x sweep 0.83 -> 0.96 ms,

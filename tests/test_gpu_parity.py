@@ -331,6 +331,26 @@ def test_real_time_huge_and_non_finite_phases(gpu, oracle):
     assert np.isnan(got[3, 4, 20].real) and np.isnan(a[3, 4, 20].real)
 
 
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("shape", [(512, 512, 20), (512, 8, 64), (8, 512, 64), (512, 12, 18)])
+def test_fft_pair_kernel_agrees(gpu, oracle, shape, mode):
+    """K2 / K3 / K4 at 512 points as k_fft_pair (two tiles per SM in different phases; the default for K3) against the
+    one-tile kernels, and both against the oracle's Phi: whole and ragged last tiles ((nz/2+1) = 11, 33, 10 bins; 12 * 10
+    = 120 flattened columns), fewer tiles than SMs and more, odd tile counts per CTA."""
+    args = (*shape, 0.3, 0.25, 0.2, 0.004, 1.0, 0.7, 1.3, 5.0, 3.0, mode)
+    psi = inputs.random_state(shape, 29) * 0.2
+    ref = oracle.Oracle(*args).dipolar(np.ascontiguousarray(psi.real ** 2 + psi.imag ** 2))
+    out = []
+    for opt in ({"tma_pair": 0}, {"tma_pair": 1}, None):
+        G = gpu.Dgpe(*args, options=opt)
+        phi = G.dipolar(dev(psi)).cpu().numpy()
+        assert np.max(np.abs(phi - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref))), opt
+        t = dev(psi)
+        G.step(t, 4)
+        out.append(t.cpu().numpy())
+    assert np.max(np.abs(out[0] - out[1])) <= 1e-13 and np.max(np.abs(out[0] - out[2])) <= 1e-13
+
+
 def test_handles_of_different_sizes_alive_together(gpu, oracle):
     """The shared-memory opt-in of a kernel is per process and device, not per handle: creating a small
     handle must not lower the limit a larger live handle launches with -- generic kernels (972 = 2^2 3^5 has no
