@@ -80,6 +80,7 @@ struct AxisSweep {
 #define DGPE_PAIR_DEFAULT_Y false
 #endif
 
+
 enum { PF_Z = 1, PF_SWEEP_Y = 2, PF_SWEEP_X = 4, PF_FFT_Y = 8, PF_FFT_X = 16 };
 
 struct dgpe_handle {
@@ -879,7 +880,9 @@ static int launch_fft_tma_xudd(dgpe_handle* h, bool* handled)
     }
 }
 
-// ---- K2 / K4 / K3 as k_fft_pair (xyfft_pair.cuh): two tiles per SM in different phases; N = 512 ----
+// ---- K2 / K4 / K3 as k_fft_pair (xyfft_pair.cuh): two tiles per SM in different phases; N = 512.
+//      (N = 768 would need 4-line tiles -- two teams of 8-line tiles are 1536 threads -- and TMA boxes with 64-byte rows
+//      measured 5x slower: K2 0.81 -> 4.4 ms, K3 1.32 -> 6.4 ms at 768 x 768 x 384) ----
 static bool fft_pair_wanted(const dgpe_handle* h, int n, bool xpass)
 {
     if (n != 512 || !h->use_tma || h->force_generic || !tensor_map_encoder()) return false;
@@ -888,12 +891,13 @@ static bool fft_pair_wanted(const dgpe_handle* h, int n, bool xpass)
     return xpass ? DGPE_PAIR_DEFAULT_X : DGPE_PAIR_DEFAULT_Y;
 }
 
-template <int N, int KIND>
+template <int N, int KIND, int COLS, int NSTAGE>
 static int launch_fft_pair(dgpe_handle* h)
 {
-    auto kern = k_fft_pair<N, KIND>;
-    const size_t smem = (size_t)3 * N * TILE_COLS * sizeof(cplx) + 128;
-    int rc = kernel_setup((const void*)kern, 2 * xy_threads<N>(), smem, nullptr);
+    auto kern = k_fft_pair<N, KIND, COLS, NSTAGE>;
+    constexpr int THREADS = 2 * pair_team_threads<N, COLS>();
+    const size_t smem = (size_t)NSTAGE * N * COLS * sizeof(cplx) + 128;
+    int rc = kernel_setup((const void*)kern, THREADS, smem, nullptr);
     if (rc) return rc;
     constexpr int nbox = tma_boxes(N);
     static_assert(nbox > 0 && N % nbox == 0 && N / nbox <= 256, "line length must split into equal TMA boxes");
@@ -903,29 +907,35 @@ static int launch_fft_pair(dgpe_handle* h)
     W.n = N; W.box_rows = N / nbox;
     if (KIND == FFT_X_UDD) {
         dims[0] = 2 * ncols; dims[1] = nx; dims[2] = 1; strides[0] = ncols * 16; strides[1] = nx * ncols * 16;
-        W.tiles_per_batch = (int)((ncols + TILE_COLS - 1) / TILE_COLS);
+        W.tiles_per_batch = (int)((ncols + COLS - 1) / COLS);
         W.ntiles = W.tiles_per_batch;
     } else {
         dims[0] = 2 * nzh; dims[1] = ny; dims[2] = nx; strides[0] = nzh * 16; strides[1] = ny * nzh * 16;
-        W.tiles_per_batch = (h->nzh + TILE_COLS - 1) / TILE_COLS;
+        W.tiles_per_batch = (h->nzh + COLS - 1) / COLS;
         W.ntiles = W.tiles_per_batch * h->nx;
     }
-    cuuint32_t box[3] = {2 * TILE_COLS, (cuuint32_t)(N / nbox), 1}, estr[3] = {1, 1, 1};
+    cuuint32_t box[3] = {2 * COLS, (cuuint32_t)(N / nbox), 1}, estr[3] = {1, 1, 1};
     CUtensorMap tmap;
     CUresult cr = tensor_map_encoder()(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, h->spec, dims, strides, box, estr,
                                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                        CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (cr != CUDA_SUCCESS) return fail(DGPE_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)cr);
     UddArgs U{h->nzh, h->kx2, h->ky2, h->kz2, 2.0 * 3.14159265358979323846264338327950288 / ((double)h->nx * h->dx), h->inv_ntot, 0};
-    kern<<<std::min(W.ntiles, h->num_sms), 2 * xy_threads<N>(), smem, h->stream>>>(tmap, W, KIND == FFT_X_UDD ? h->tw_x : h->tw_y, U, (int)ncols);
+    kern<<<std::min(W.ntiles, h->num_sms), THREADS, smem, h->stream>>>(tmap, W, KIND == FFT_X_UDD ? h->tw_x : h->tw_y, U, (int)ncols);
     return check_launch("k_fft_pair");
+}
+
+template <int KIND>
+static int launch_fft_pair_n(dgpe_handle* h, int)
+{
+    return launch_fft_pair<512, KIND, 8, 3>(h);
 }
 
 static int launch_fft_y(dgpe_handle* h, bool inverse)
 {
     const int nx = h->nx, ny = h->ny, nzh = h->nzh;
     LineMap my{ny, nzh, (long long)ny * nzh, 1, nzh};
-    if (fft_pair_wanted(h, ny, false)) return inverse ? launch_fft_pair<512, FFT_INV>(h) : launch_fft_pair<512, FFT_FWD>(h);
+    if (fft_pair_wanted(h, ny, false)) return inverse ? launch_fft_pair_n<FFT_INV>(h, ny) : launch_fft_pair_n<FFT_FWD>(h, ny);
     if (!h->force_generic) {
         bool handled = false;
         int rct = launch_fft_tma(h, inverse, &handled);
@@ -962,7 +972,7 @@ static int launch_fft_x_udd(dgpe_handle* h)
 {
     const int nx = h->nx, ny = h->ny, nzh = h->nzh;
     LineMap mx{nx, ny * nzh, 0, 1, (long long)ny * nzh};
-    if (fft_pair_wanted(h, nx, true)) return launch_fft_pair<512, FFT_X_UDD>(h);
+    if (fft_pair_wanted(h, nx, true)) return launch_fft_pair_n<FFT_X_UDD>(h, nx);
     if (!h->force_generic) {
         bool handled = false;
         int rc = launch_fft_tma_xudd(h, &handled);

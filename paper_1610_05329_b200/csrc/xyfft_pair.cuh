@@ -10,7 +10,10 @@
 // The leader of the half that finished tile t-2 refills that stage with tile t+1 (which the OTHER half will consume)
 // once its store has been read; arrival is signalled on the stage's mbarrier as in k_fft_tma.
 //
-// Lengths: 2 xy_threads<N>() <= 1024 threads and 3 N 128 bytes <= 227 KB: N = 384, 480, 512.
+// COLS = lines per tile (8: 128-byte rows).  Used at N = 512.  At N = 768 two teams of 8-line tiles would need 1536
+// threads; with COLS = 4 (64-byte rows) the TMA moves the tiles five times slower (measured), and
+// N = 384, 480 (radix-3/5 passes) spill 1-2 KB per thread inside the 64-register budget of a 1024-thread CTA.
+// Constraints: 2 COLS N / rmax(N) <= 1024 threads, NSTAGE N COLS 16 bytes <= 227 KB, <= 64 registers per butterfly.
 #pragma once
 #include "xyfft_tma.cuh"
 
@@ -26,24 +29,32 @@ struct SyncHalf {
 
 // KIND = FFT_FWD / FFT_INV: transform along y, tensor map {2 (nz/2+1), ny, nx}; KIND = FFT_X_UDD: FFT along x, Udd~(k)/N,
 // inverse FFT along x, tensor map {2 ny (nz/2+1), nx, 1} (as k_fft_tma / k_fft_tma_xudd).
-// grid = min(ceil(ntiles / 2), #SMs); block = 2 xy_threads<N>(); dynamic smem = 3 N 128 bytes (+128)
-template <int N, int KIND>
-__global__ void __launch_bounds__(2 * xy_threads<N>(), 1)
+template <int COLS>
+struct PosCols {
+    static __device__ __forceinline__ int at(int idx) { return idx * COLS; }
+};
+template <int N, int COLS>
+__host__ __device__ constexpr int pair_team_threads() { return (COLS * xy_nbf<N>() + 31) / 32 * 32; }
+
+// grid = min(ntiles, #SMs); block = 2 pair_team_threads<N, COLS>(); dynamic smem = NSTAGE N COLS 16 bytes (+128)
+// W.tiles_per_batch / W.ntiles count tiles of COLS lines.
+template <int N, int KIND, int COLS, int NSTAGE>
+__global__ void __launch_bounds__(2 * pair_team_threads<N, COLS>(), 1)
 k_fft_pair(const __grid_constant__ CUtensorMap tmap, TmaWalk W, const cplx* __restrict__ tw, UddArgs U, int ncols)
 {
-    constexpr int HT = xy_threads<N>();
+    constexpr int HT = pair_team_threads<N, COLS>();
     constexpr int NBF = xy_nbf<N>();
     constexpr int L = ct::npass(N);
-    constexpr int NSTAGE = 3;
     constexpr bool INV = KIND == FFT_INV;
+    using PosTile = PosCols<COLS>;
     using Sync = SyncHalf<HT>;
     static_assert(L >= 2 && 2 * HT <= 1024, "two halves of a CTA");
     extern __shared__ unsigned char smem_dyn[];
     __shared__ __align__(8) unsigned long long full[NSTAGE];
     cplx* stages = reinterpret_cast<cplx*>(smem_dyn + ((128u - (smem_addr(smem_dyn) & 127u)) & 127u));
-    constexpr int tile_elems = N * TILE_COLS;
+    constexpr int tile_elems = N * COLS;
     constexpr unsigned tile_bytes = (unsigned)tile_elems * 16u;
-    const int half = threadIdx.x / HT, tid = threadIdx.x - half * HT, c = tid & 7, b = tid >> 3;
+    const int half = threadIdx.x / HT, tid = threadIdx.x - half * HT, c = tid % COLS, b = tid / COLS;
     const bool on = b < NBF;
     const int first = blockIdx.x, stride = gridDim.x;
     const int nmine = (first < W.ntiles) ? (W.ntiles - first + stride - 1) / stride : 0;
@@ -51,11 +62,11 @@ k_fft_pair(const __grid_constant__ CUtensorMap tmap, TmaWalk W, const cplx* __re
     auto coords = [&](int it, int& c0, int& c2) {
         const int t = first + it * stride;
         if constexpr (KIND == FFT_X_UDD) {
-            c0 = t * (2 * TILE_COLS);
+            c0 = t * (2 * COLS);
             c2 = 0;
         } else {
             const int bat = t / W.tiles_per_batch;
-            c0 = (t - bat * W.tiles_per_batch) * (2 * TILE_COLS);
+            c0 = (t - bat * W.tiles_per_batch) * (2 * COLS);
             c2 = bat;
         }
     };
@@ -65,7 +76,7 @@ k_fft_pair(const __grid_constant__ CUtensorMap tmap, TmaWalk W, const cplx* __re
         const int st = it % NSTAGE;
         mbar_expect_tx(&full[st], tile_bytes);
         for (int r0 = 0; r0 < N; r0 += W.box_rows)
-            tma_load_3d(stages + (size_t)st * tile_elems + (size_t)r0 * TILE_COLS, &tmap, c0, r0, c2, &full[st]);
+            tma_load_3d(stages + (size_t)st * tile_elems + (size_t)r0 * COLS, &tmap, c0, r0, c2, &full[st]);
     };
 
     if (threadIdx.x == 0) {
@@ -85,7 +96,7 @@ k_fft_pair(const __grid_constant__ CUtensorMap tmap, TmaWalk W, const cplx* __re
         double qy = 0.0, qz = 0.0;
         if constexpr (KIND == FFT_X_UDD) {
             // ky^2, kz^2 of this thread's column (columns past the end of a ragged last tile take the last column's)
-            const int cidx = min((first + it * stride) * TILE_COLS + c, ncols - 1);
+            const int cidx = min((first + it * stride) * COLS + c, ncols - 1);
             const int ky = cidx / U.nzh, kz = cidx - ky * U.nzh;
             qy = __ldg(&U.ky2[ky]);
             qz = __ldg(&U.kz2[kz]);
@@ -93,16 +104,16 @@ k_fft_pair(const __grid_constant__ CUtensorMap tmap, TmaWalk W, const cplx* __re
         mbar_wait(&full[st], (unsigned)((it / NSTAGE) & 1));
 
         // pass 0 by hand: after its barrier this half's leader refills the stage of the half's previous tile (it - 2),
-        // which is the stage of tile it + 1 -- the other half's next tile
+        // which is the stage of tile it - 2 + NSTAGE (with three stages: the other half's next tile)
         CtPass<N, 0, INV, false, NBF> p0;
         if (on) {
             if constexpr (KIND == FFT_X_UDD) p0.load_tw(b, tw);
             p0.load(b, [&](int idx) { return col[PosTile::at(idx)]; });
         }
         Sync::sync();                                    // every read of pass 0 precedes its writes
-        if (tid == 0 && it >= 2 && it + 1 < nmine) {
+        if (tid == 0 && it >= 2 && it - 2 + NSTAGE < nmine) {
             tma_store_wait_read<0>();                    // my store of tile it - 2 has read its stage
-            issue_load(it + 1);
+            issue_load(it - 2 + NSTAGE);
         }
         if (on) {
             p0.bfly(b);
@@ -163,7 +174,7 @@ k_fft_pair(const __grid_constant__ CUtensorMap tmap, TmaWalk W, const cplx* __re
         if (tid == 0) {
             int c0, c2;
             coords(it, c0, c2);
-            for (int r0 = 0; r0 < N; r0 += W.box_rows) tma_store_3d(&tmap, c0, r0, c2, tile + (size_t)r0 * TILE_COLS);
+            for (int r0 = 0; r0 < N; r0 += W.box_rows) tma_store_3d(&tmap, c0, r0, c2, tile + (size_t)r0 * COLS);
             tma_store_commit();
         }
     }
