@@ -78,8 +78,12 @@ __device__ __forceinline__ cplx ct_zero(cplx) { return mk(0.0, 0.0); }
 // ------------------------------------------------------------------------------------------------
 // DT = cplx: psi is complex (16 bytes per point); DT = double: real-valued psi of the imaginary-time
 // fast path (SV section 8f NEXT-2; 8 bytes per point, n = s2 psi^2).
+// resident CTAs per SM the register budget of K1 is tuned for: 32 lines (64 registers) pay at nz = 384 (C5: 1.09 -> 0.98 ms);
+// at nz = 256, 480, 512 the 28 lines of the compiler's own 68-72 registers are faster (512^3: 0.515 vs 0.553 ms)
+template <int NZ>
+__host__ __device__ constexpr int k1_min_ctas() { return NZ == 384 ? 32 : 28; }
 template <int NZ, int WARPS, typename DT>
-__global__ void __launch_bounds__(32 * WARPS)
+__global__ void __launch_bounds__(32 * WARPS, k1_min_ctas<NZ>())
 k_z_r2c(const DT* __restrict__ psi, cplx* __restrict__ spec, int nlines, const cplx* __restrict__ tw,
         const cplx* __restrict__ tws, const double* __restrict__ scal)
 {
