@@ -32,7 +32,8 @@ def gather(slabs):
 # (shape, ranks): cubic and non-cubic, z-line kernels (nz = 64, 128) and generic z (nz = 20, 36), radix 3 and 5,
 # thin slabs (nx/P = 2), TMA-sized lines (384, 512) next to short ones
 CASES = [((16, 16, 16), 1), ((16, 16, 16), 2), ((16, 16, 16), 4), ((64, 32, 64), 4), ((48, 96, 20), 3), ((30, 20, 36), 5),
-         ((32, 64, 128), 8), ((384, 16, 64), 2), ((16, 512, 64), 4)]
+         ((32, 64, 128), 8), ((384, 16, 64), 2), ((16, 512, 64), 4),
+         ((512, 16, 64), 2)]           # nx = 512: the x pass of the y-slab view runs as k_fft_pair
 
 
 @pytest.mark.parametrize("shape,P", CASES)
