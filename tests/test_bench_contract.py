@@ -34,3 +34,21 @@ def test_traffic_table_names_the_kernels_of_the_step():
     assert bench.ncu_traffic("no such kernel") is None
     peak, src = bench.load_peaks()
     assert 3000 < peak < 9000 and ("measured" in src or "fallback" in src)
+
+
+def test_committed_ncu_tables_pair_the_step_kernels_with_the_right_cuda_kernels():
+    """profiles/r2_*_ncu_full.md pairs the kernels of a step (bench.py names) with ncu's launches by ORDER: a kernel missing
+    from the ncu filter shifts every row after it (it happened once).  Each row must name the kernel family of its stage."""
+    import glob
+    want = {"K1": "k_z_r2c", "K2": "k_fft", "K3": "k_fft", "K4": "k_fft", "K5+K8": "k_z_main", "K6": "k_sweep", "K7": "k_sweep"}
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r2_*_ncu_full.md")))
+    assert len(files) >= 3
+    for path in files:
+        rows = [l for l in open(path) if l.startswith("| K")]
+        assert len(rows) == 7, path
+        for line in rows:
+            cells = [c.strip() for c in line.split("|")]
+            stage, kernel = cells[1].split(" ")[0], cells[2]
+            assert want[stage] in kernel, (path, stage, kernel)
+            algorithmic, read, write = float(cells[6]), float(cells[4]), float(cells[5])
+            assert 0.9 * algorithmic <= read + write <= 1.15 * algorithmic, (path, stage, read, write, algorithmic)
