@@ -52,3 +52,16 @@ def test_committed_ncu_tables_pair_the_step_kernels_with_the_right_cuda_kernels(
             assert want[stage] in kernel, (path, stage, kernel)
             algorithmic, read, write = float(cells[6]), float(cells[4]), float(cells[5])
             assert 0.9 * algorithmic <= read + write <= 1.15 * algorithmic, (path, stage, read, write, algorithmic)
+
+
+def test_measured_full_size_oracle_step_comes_from_the_golden_headers():
+    """bench.py's cpu_baseline.measured_full_size_s_per_step is the oracle's measured time for one FULL-SIZE step, recorded in
+    the headers of the goldens the oracle wrote offline (tests/golden/make_fullsize_goldens.py)."""
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1610_05329_b200 import inputs
+    c4 = bench.measured_full_size(inputs.CONFIGS["C4"])
+    c2 = bench.measured_full_size(inputs.CONFIGS["C2"])
+    assert c4 is not None and 60.0 < c4 < 1000.0            # 512^3: minutes per step on one core
+    assert c2 is not None and 0.5 < c2 < 30.0 and c2 < c4   # 128^3: seconds
+    assert bench.measured_full_size(inputs.CONFIGS["C1"]) is None      # no full-size golden run for C1 (the tests run it live)
