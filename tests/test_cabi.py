@@ -79,3 +79,16 @@ def test_product_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src and "dgpe_oracle" not in src, f
+
+
+def test_header_is_plain_c():
+    """The boundary is a C ABI: include/dgpe.h must compile as C99 (no C++-only constructs, no torch or CUDA types)."""
+    import shutil
+    import subprocess
+    if not shutil.which("gcc"):
+        pytest.skip("gcc not found")
+    hdr = os.path.join(ROOT, "include", "dgpe.h")
+    res = subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-fsyntax-only", "-x", "c", hdr], capture_output=True, text=True)
+    assert res.returncode == 0, res.stderr
+    code = re.sub(r"/\*.*?\*/", "", open(hdr).read(), flags=re.S)        # the declarations, comments stripped
+    assert "torch" not in code and "cudaStream_t" not in code and "#include" not in code
